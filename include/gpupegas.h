@@ -1,0 +1,115 @@
+/*
+ * include/gpupegas.h — C ABI of libgpupegas.so: the B200 (sm_100a) hot path of GPUPEGAS
+ * (I. Kulikov, arXiv:1311.0861): one explicit fp64 timestep of the operator-split
+ * Godunov + FIIC (fluids-in-cell) scheme on a uniform 3-D Cartesian grid, for a gas and a
+ * collisionless component, with an FFT Poisson solve and a CFL reduction.
+ *
+ * Everything behind these calls runs in hand-written CUDA kernels (plus cuFFT for the
+ * transforms).  There is no CPU fallback: without a CUDA device gp_create fails.
+ *
+ * Conventions
+ *   - Every int-returning call returns GP_OK or an error code and never throws; the text of
+ *     the last error of the calling thread is available from gp_last_error().
+ *   - A field is nx*ny*nz contiguous doubles, x fastest (c = i + nx*(j + ny*k)), interior
+ *     cells only: ghost cells never cross the ABI (they are index maps inside the kernels).
+ *   - Pointers passed in stay owned by the caller; the library copies.  `*_on_device` says
+ *     whether such a pointer is device memory (non-zero) or host memory (0).
+ *   - Work is issued asynchronously on the context's stream (default: the legacy default
+ *     stream; see gp_set_stream).  Calls that hand a result to the host (gp_get_state to a
+ *     host pointer, gp_max_dt with dt != NULL) synchronise that stream.
+ *   - Cubic cells only (one h).  nx, ny, nz >= 4.  With a Poisson mode, nx, ny, nz even.
+ *   - One "full timestep" of the metric = gp_max_dt + gp_solve_poisson (if gravity) + gp_step.
+ */
+#ifndef GPUPEGAS_H
+#define GPUPEGAS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gp_ctx gp_ctx;   /* opaque; created by gp_create, freed by gp_destroy */
+
+enum { GP_OK = 0, GP_ERR_ARG = 1, GP_ERR_ALLOC = 2, GP_ERR_CUDA = 3, GP_ERR_CUFFT = 4,
+       GP_ERR_STATE = 5 /* NaN/Inf, or rho, n, p or Pi_dd <= 0 seen */, GP_ERR_UNSUPPORTED = 6 };
+
+enum { GP_GAS = 1, GP_STARS = 2 };                                  /* components bit mask */
+enum { GP_POISSON_NONE = 0, GP_POISSON_PERIODIC = 1, GP_POISSON_ISOLATED = 2 };
+enum { GP_BC_PERIODIC = 0, GP_BC_OUTFLOW = 1 };
+
+/* Conserved fields.  Gas: rho, rho*v (3), rho*E.  Collisionless component
+ * (PAPER.md:57, 63): n, n*u (3), n*E_ij (6, symmetric: xx xy xz yy yz zz).  Potential
+ * (PAPER.md:186): Phi + Phi0, one field for the summed density. */
+enum { GP_RHO = 0, GP_MX, GP_MY, GP_MZ, GP_E,
+       GP_N, GP_NUX, GP_NUY, GP_NUZ, GP_EXX, GP_EXY, GP_EXZ, GP_EYY, GP_EYZ, GP_EZZ,
+       GP_PHI, GP_NFIELDS };
+
+typedef struct {
+    int nx, ny, nz;      /* interior cells per axis */
+    double h;            /* cell size (with h_x = h_y = h_z) */
+    int components;      /* GP_GAS | GP_STARS */
+    int poisson;         /* GP_POISSON_* */
+    double G;            /* gravitational constant multiplying the source of PAPER.md:186 */
+} gp_grid;
+
+typedef struct { int x, y, z; } gp_bc;   /* GP_BC_* per axis, applied to the hydro fields */
+
+/* Create a context for `grid`, adiabatic index `gamma` and boundary rule `bc`.
+ * Allocates nothing large: device storage is taken at the first call that needs it, from the
+ * region bound with gp_bind_storage if there is one, else with cudaMalloc.  Returns NULL on
+ * failure (bad arguments, no CUDA device). */
+gp_ctx* gp_create(const gp_grid* grid, double gamma, const gp_bc* bc);
+void gp_destroy(gp_ctx* ctx);
+
+/* Copy one field in / out.  `field` must belong to an enabled component (or be GP_PHI), else
+ * GP_ERR_ARG.  Setting GP_PHI also fills its ghost faces by the hydro boundary rule. */
+int gp_set_state(gp_ctx* ctx, int field, const double* src, int src_on_device);
+int gp_get_state(gp_ctx* ctx, int field, double* dst, int dst_on_device);
+
+/* Phi <- solution of the Poisson equation for (rho + n) of the current state.
+ * Periodic mode: PAPER.md:190 (exact inverse of the 27-point Laplacian, zero-mean Phi).
+ * Isolated mode: zero-padded (2N)^3 convolution with the -G/r kernel (Hockney & Eastwood).
+ * GP_POISSON_NONE: GP_ERR_UNSUPPORTED. */
+int gp_solve_poisson(gp_ctx* ctx);
+
+/* CFL reduction: dt = cfl*h / max over cells and axes of (|v_d| + sqrt(gamma p/rho)) and
+ * (|u_d| + sqrt(3 Pi_dd/n)) (wave speeds PAPER.md:86, 140).  The result stays on the device
+ * for gp_step(ctx, 0).  If `dt` is not NULL the call also copies it to *dt (host pointer),
+ * synchronises, and returns GP_ERR_STATE if the state holds NaN/Inf or a non-positive
+ * rho, n, p or Pi_dd. */
+int gp_max_dt(gp_ctx* ctx, double cfl, double* dt);
+
+/* One timestep: Eulerian stage (face values PAPER.md:112-114 and
+ * 170-178, pressure and gravity sources from the stored Phi) then Lagrangian stage (upwind
+ * flux-form advection), for every enabled component.  dt > 0: use it; dt <= 0: use the
+ * device-resident dt of the last gp_max_dt. */
+int gp_step(gp_ctx* ctx, double dt);
+
+const char* gp_last_error(void);   /* thread-local static text; never freed by the caller */
+
+/* ---- optional: let the caller (e.g. PyTorch) own the stream and the device memory ---- */
+int gp_set_stream(gp_ctx* ctx, void* cuda_stream);          /* a cudaStream_t; NULL = default stream */
+size_t gp_storage_bytes(const gp_grid* grid);               /* size of the state + work storage */
+/* Hand the context a device region of at least gp_storage_bytes(grid) bytes, 256-byte aligned.
+ * Must be called before the first call that touches device state.  The caller keeps ownership
+ * and must keep it alive until gp_destroy. */
+int gp_bind_storage(gp_ctx* ctx, void* device_ptr, size_t bytes);
+int gp_synchronize(gp_ctx* ctx);                            /* wait for the context's stream */
+/* Number of kernel launches (own kernels and cuFFT executions counted separately) issued by this
+ * context so far; for the bench's gpu_launches claim. */
+int gp_launch_counts(gp_ctx* ctx, long long* own_kernels, long long* cufft_execs);
+
+/* ---- optional: per-kernel timing with CUDA events on the context's stream ----
+ * gp_timing_enable(ctx, 1) zeroes the totals and brackets every later kernel launch (and cuFFT
+ * execution) with an event pair; gp_timing_enable(ctx, 0) stops.  gp_timing_read synchronises
+ * the stream and returns, per kernel kind that ran, its name (static string), the summed
+ * elapsed milliseconds and the number of launches; at most max_entries entries are written. */
+int gp_timing_enable(gp_ctx* ctx, int on);
+int gp_timing_read(gp_ctx* ctx, int max_entries, int* n_entries, const char** names, double* total_ms,
+                   long long* launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

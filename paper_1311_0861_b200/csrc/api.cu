@@ -1,0 +1,338 @@
+// C ABI of libgpupegas.so (include/gpupegas.h): context, storage, field copies, and the
+// sequencing of the kernels of one timestep.  No torch types, no CPU fallback.
+#include <cstdarg>
+#include <cstring>
+#include <new>
+
+#include "gp_internal.h"
+
+namespace gp {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+static const char* const kKernelNames[K_NUM] = {
+    "eulerian_gas", "lagrangian_gas", "eulerian_bme", "lagrangian_bme", "cfl", "poisson_source", "cufft_forward",
+    "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract"};
+
+void tic(gp_ctx* c, int kid) {
+    Timing* t = c->tim;
+    if (!t || !t->on) return;
+    if (t->used == t->cap) {
+        const size_t ncap = t->cap ? 2 * t->cap : 256;
+        cudaEvent_t* ev = new cudaEvent_t[2 * ncap];
+        int* kd = new int[ncap];
+        for (size_t i = 0; i < 2 * t->cap; ++i) ev[i] = t->ev[i];
+        for (size_t i = 0; i < t->cap; ++i) kd[i] = t->kid[i];
+        for (size_t i = 2 * t->cap; i < 2 * ncap; ++i) cudaEventCreate(&ev[i]);
+        delete[] t->ev; delete[] t->kid;
+        t->ev = ev; t->kid = kd; t->cap = ncap;
+    }
+    t->kid[t->used] = kid;
+    cudaEventRecord(t->ev[2 * t->used], c->stream);
+}
+
+void toc(gp_ctx* c) {
+    Timing* t = c->tim;
+    if (!t || !t->on) return;
+    cudaEventRecord(t->ev[2 * t->used + 1], c->stream);
+    t->used++;
+}
+
+static void timing_collect(gp_ctx* c) {
+    Timing* t = c->tim;
+    if (!t) return;
+    cudaStreamSynchronize(c->stream);
+    for (size_t i = 0; i < t->used; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, t->ev[2 * i], t->ev[2 * i + 1]) == cudaSuccess) {
+            t->ms[t->kid[i]] += ms;
+            t->cnt[t->kid[i]]++;
+        }
+    }
+    t->used = 0;
+}
+
+static bool field_enabled(const gp_grid& g, int f) {
+    if (f == GP_PHI) return true;
+    if (f < 0 || f >= GP_NFIELDS) return false;
+    return f < NGAS ? (g.components & GP_GAS) != 0 : (g.components & GP_STARS) != 0;
+}
+
+static size_t ghost_elems(const gp_grid& g) {
+    return 2 * ((size_t)g.ny * g.nz + (size_t)g.nx * g.nz + (size_t)g.nx * g.ny);
+}
+
+static size_t storage_bytes(const gp_grid& g) {
+    const size_t N = (size_t)g.nx * g.ny * g.nz;
+    const size_t fb = align256(N * sizeof(double));
+    size_t nf = 0;
+    if (g.components & GP_GAS) nf += NGAS;
+    if (g.components & GP_STARS) nf += NBME;
+    size_t b = (2 * nf + 3 + 1) * fb;                 // U, U*, w*, Phi
+    b += 6 * align256(ghost_elems(g) / 2 * sizeof(double));   // generous: each face <= half of the total
+    b += 256;                                         // dt, smax, flag
+    b += poisson_storage_bytes(&g);
+    return b;
+}
+
+// Carve the bound (or freshly allocated) region.
+static int ensure_storage(gp_ctx* c) {
+    if (c->ready) return GP_OK;
+    const gp_grid& g = c->g;
+    const size_t need = storage_bytes(g);
+    if (!c->base) {
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, need);
+        if (e != cudaSuccess) {
+            set_error("cudaMalloc of %zu bytes failed: %s", need, cudaGetErrorString(e));
+            return GP_ERR_ALLOC;
+        }
+        c->base = (char*)p;
+        c->bytes = need;
+        c->owns = true;
+    } else if (c->bytes < need) {
+        set_error("bound storage too small: %zu < %zu", c->bytes, need);
+        return GP_ERR_ARG;
+    }
+    char* p = c->base;
+    auto take = [&](size_t bytes) { char* r = p; p += align256(bytes); return r; };
+    const size_t N = c->N;
+    for (int f = 0; f < NHYD; ++f) {
+        c->U[f] = c->Us[f] = nullptr;
+        if (field_enabled(g, f)) {
+            c->U[f] = (double*)take(N * sizeof(double));
+            c->Us[f] = (double*)take(N * sizeof(double));
+        }
+    }
+    for (int d = 0; d < 3; ++d) c->W[d] = (double*)take(N * sizeof(double));
+    c->phi = (double*)take(N * sizeof(double));
+    const size_t face[3] = {(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny};
+    for (int s = 0; s < 6; ++s) c->phig[s] = (double*)take(face[s / 2] * sizeof(double));
+    char* small = take(256);
+    c->d_dt = (double*)small;
+    c->d_smax = (unsigned long long*)(small + 64);
+    c->d_flag = (int*)(small + 128);
+    c->spec = nullptr; c->padded = nullptr; c->kspec = nullptr; c->tabx = c->taby = c->tabz = nullptr;
+    if (g.poisson == GP_POISSON_PERIODIC) {
+        c->spec = (cufftDoubleComplex*)take(((size_t)g.nx / 2 + 1) * g.ny * g.nz * sizeof(cufftDoubleComplex));
+        c->tabx = (double*)take(((size_t)g.nx + g.ny + g.nz) * sizeof(double));
+        c->taby = c->tabx + g.nx;
+        c->tabz = c->taby + g.ny;
+    } else if (g.poisson == GP_POISSON_ISOLATED) {
+        const size_t half = ((size_t)g.nx + 1) * (2 * (size_t)g.ny) * (2 * (size_t)g.nz);
+        c->spec = (cufftDoubleComplex*)take(half * sizeof(cufftDoubleComplex));
+        c->kspec = (double*)take(half * sizeof(double));
+        c->padded = (double*)take(8 * N * sizeof(double));
+    }
+    if ((size_t)(p - c->base) > c->bytes) {
+        set_error("internal: storage layout (%zu) exceeds the region (%zu)", (size_t)(p - c->base), c->bytes);
+        return GP_ERR_ALLOC;
+    }
+    // zero state, Phi and its ghost faces (GP_POISSON_NONE with Phi never set means no gravity)
+    GP_CUDA(cudaMemsetAsync(c->base, 0, (size_t)(p - c->base), c->stream));
+    c->ready = true;
+    return GP_OK;
+}
+
+}  // namespace gp
+
+using namespace gp;
+
+extern "C" {
+
+const char* gp_last_error(void) { return g_err; }
+
+gp_ctx* gp_create(const gp_grid* grid, double gamma, const gp_bc* bc) {
+    if (!grid || !bc) { set_error("gp_create: NULL argument"); return nullptr; }
+    if (grid->nx < 4 || grid->ny < 4 || grid->nz < 4 || !(grid->h > 0.0)) {
+        set_error("gp_create: need nx, ny, nz >= 4 and h > 0");
+        return nullptr;
+    }
+    if (!(grid->components & (GP_GAS | GP_STARS)) || (grid->components & ~(GP_GAS | GP_STARS))) {
+        set_error("gp_create: components must be GP_GAS, GP_STARS or both");
+        return nullptr;
+    }
+    if (grid->poisson < GP_POISSON_NONE || grid->poisson > GP_POISSON_ISOLATED) { set_error("gp_create: bad poisson mode"); return nullptr; }
+    if (grid->poisson != GP_POISSON_NONE && ((grid->nx | grid->ny | grid->nz) & 1)) {
+        set_error("gp_create: Poisson modes need even nx, ny, nz");
+        return nullptr;
+    }
+    const int b[3] = {bc->x, bc->y, bc->z};
+    for (int d = 0; d < 3; ++d)
+        if (b[d] != GP_BC_PERIODIC && b[d] != GP_BC_OUTFLOW) { set_error("gp_create: bad boundary code"); return nullptr; }
+    if (!(gamma > 1.0)) { set_error("gp_create: gamma must exceed 1"); return nullptr; }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) {
+        set_error("gp_create: no CUDA device (%s); this library has no CPU path", cudaGetErrorString(e));
+        return nullptr;
+    }
+    gp_ctx* c = new (std::nothrow) gp_ctx;
+    if (!c) { set_error("gp_create: out of host memory"); return nullptr; }
+    std::memset((void*)c, 0, sizeof(*c));
+    c->g = *grid;
+    c->gamma = gamma;
+    c->bc = *bc;
+    c->N = (size_t)grid->nx * grid->ny * grid->nz;
+    c->stream = nullptr;
+    return c;
+}
+
+void gp_destroy(gp_ctx* c) {
+    if (!c) return;
+    if (c->ready || c->fft_ready) cudaStreamSynchronize(c->stream);
+    poisson_teardown(c);
+    if (c->owns && c->base) cudaFree(c->base);
+    if (c->tim) {
+        for (size_t i = 0; i < 2 * c->tim->cap; ++i) cudaEventDestroy(c->tim->ev[i]);
+        delete[] c->tim->ev; delete[] c->tim->kid;
+        delete c->tim;
+    }
+    delete c;
+}
+
+int gp_set_stream(gp_ctx* c, void* stream) {
+    if (!c) { set_error("gp_set_stream: NULL context"); return GP_ERR_ARG; }
+    if (c->ready) GP_CUDA(cudaStreamSynchronize(c->stream));
+    c->stream = (cudaStream_t)stream;
+    if (c->fft_ready) {
+        GP_CUFFT(cufftSetStream(c->plan_fwd, c->stream));
+        GP_CUFFT(cufftSetStream(c->plan_inv, c->stream));
+    }
+    return GP_OK;
+}
+
+size_t gp_storage_bytes(const gp_grid* grid) {
+    if (!grid) return 0;
+    return storage_bytes(*grid);
+}
+
+int gp_bind_storage(gp_ctx* c, void* device_ptr, size_t bytes) {
+    if (!c || !device_ptr) { set_error("gp_bind_storage: NULL argument"); return GP_ERR_ARG; }
+    if (c->ready || c->base) { set_error("gp_bind_storage: storage already in use"); return GP_ERR_ARG; }
+    if (((size_t)device_ptr & 255) != 0) { set_error("gp_bind_storage: pointer must be 256-byte aligned"); return GP_ERR_ARG; }
+    if (bytes < storage_bytes(c->g)) { set_error("gp_bind_storage: %zu bytes given, %zu needed", bytes, storage_bytes(c->g)); return GP_ERR_ARG; }
+    c->base = (char*)device_ptr;
+    c->bytes = bytes;
+    c->owns = false;
+    return GP_OK;
+}
+
+int gp_synchronize(gp_ctx* c) {
+    if (!c) { set_error("gp_synchronize: NULL context"); return GP_ERR_ARG; }
+    GP_CUDA(cudaStreamSynchronize(c->stream));
+    return GP_OK;
+}
+
+int gp_launch_counts(gp_ctx* c, long long* own, long long* fft) {
+    if (!c) { set_error("gp_launch_counts: NULL context"); return GP_ERR_ARG; }
+    if (own) *own = c->n_own;
+    if (fft) *fft = c->n_fft;
+    return GP_OK;
+}
+
+int gp_timing_enable(gp_ctx* c, int on) {
+    if (!c) { set_error("gp_timing_enable: NULL context"); return GP_ERR_ARG; }
+    if (!c->tim) c->tim = new (std::nothrow) Timing;
+    if (!c->tim) { set_error("gp_timing_enable: out of host memory"); return GP_ERR_ALLOC; }
+    timing_collect(c);
+    if (on && !c->tim->on) {
+        for (int k = 0; k < K_NUM; ++k) { c->tim->ms[k] = 0.0; c->tim->cnt[k] = 0; }
+    }
+    c->tim->on = on != 0;
+    return GP_OK;
+}
+
+int gp_timing_read(gp_ctx* c, int max_entries, int* n_entries, const char** names, double* total_ms, long long* launches) {
+    if (!c || !n_entries) { set_error("gp_timing_read: NULL argument"); return GP_ERR_ARG; }
+    *n_entries = 0;
+    if (!c->tim) return GP_OK;
+    timing_collect(c);
+    int n = 0;
+    for (int k = 0; k < K_NUM && n < max_entries; ++k) {
+        if (!c->tim->cnt[k]) continue;
+        if (names) names[n] = kKernelNames[k];
+        if (total_ms) total_ms[n] = c->tim->ms[k];
+        if (launches) launches[n] = c->tim->cnt[k];
+        ++n;
+    }
+    *n_entries = n;
+    return GP_OK;
+}
+
+int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
+    if (!c || !src) { set_error("gp_set_state: NULL argument"); return GP_ERR_ARG; }
+    if (!field_enabled(c->g, field)) { set_error("gp_set_state: field %d is not enabled", field); return GP_ERR_ARG; }
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    double* dst = field == GP_PHI ? c->phi : c->U[field];
+    GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));   // the host buffer may be reused on return
+    if (field == GP_PHI) return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
+    return GP_OK;
+}
+
+int gp_get_state(gp_ctx* c, int field, double* dst, int on_device) {
+    if (!c || !dst) { set_error("gp_get_state: NULL argument"); return GP_ERR_ARG; }
+    if (!field_enabled(c->g, field)) { set_error("gp_get_state: field %d is not enabled", field); return GP_ERR_ARG; }
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    const double* src = field == GP_PHI ? c->phi : c->U[field];
+    GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));
+    return GP_OK;
+}
+
+int gp_solve_poisson(gp_ctx* c) {
+    if (!c) { set_error("gp_solve_poisson: NULL context"); return GP_ERR_ARG; }
+    if (c->g.poisson == GP_POISSON_NONE) { set_error("gp_solve_poisson: context was created with GP_POISSON_NONE"); return GP_ERR_UNSUPPORTED; }
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    return poisson_solve(c);
+}
+
+int gp_max_dt(gp_ctx* c, double cfl, double* dt) {
+    if (!c || !(cfl > 0.0)) { set_error("gp_max_dt: bad argument"); return GP_ERR_ARG; }
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    rc = launch_cfl(c, cfl);
+    if (rc != GP_OK) return rc;
+    if (dt) {
+        double h_dt = 0.0;
+        int h_flag = 0;
+        GP_CUDA(cudaMemcpyAsync(&h_dt, c->d_dt, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        GP_CUDA(cudaMemcpyAsync(&h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        GP_CUDA(cudaStreamSynchronize(c->stream));
+        *dt = h_dt;
+        if (h_flag) { set_error("gp_max_dt: state holds NaN/Inf or a non-positive rho, n, p or Pi_dd"); return GP_ERR_STATE; }
+    }
+    return GP_OK;
+}
+
+int gp_step(gp_ctx* c, double dt) {
+    if (!c) { set_error("gp_step: NULL context"); return GP_ERR_ARG; }
+    if (dt != dt) { set_error("gp_step: dt is NaN"); return GP_ERR_ARG; }
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    const double* d_dt = dt > 0.0 ? nullptr : c->d_dt;
+    if (c->g.components & GP_GAS) {
+        if ((rc = launch_eulerian_gas(c, dt, d_dt)) != GP_OK) return rc;
+        if ((rc = launch_lagrangian(c, 0, NGAS, dt, d_dt)) != GP_OK) return rc;
+    }
+    if (c->g.components & GP_STARS) {
+        if ((rc = launch_eulerian_bme(c, dt, d_dt)) != GP_OK) return rc;
+        if ((rc = launch_lagrangian(c, NGAS, NBME, dt, d_dt)) != GP_OK) return rc;
+    }
+    return GP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,131 @@
+// Internal declarations shared by the translation units of libgpupegas.so (CUDA path only;
+// nothing here is seen by oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <cstddef>
+#include <cstdio>
+
+#include "../../include/gpupegas.h"
+
+namespace gp {
+
+constexpr int NGAS = 5;
+constexpr int NBME = 10;
+constexpr int NHYD = NGAS + NBME;
+
+// Grid geometry handed to kernels by value.
+struct Geo {
+    int nx, ny, nz;
+    int bcx, bcy, bcz;
+};
+
+// Field pointer bundles (kernel arguments).
+template <int NF>
+struct Fields {
+    double* p[NF];
+};
+template <int NF>
+struct ConstFields {
+    const double* p[NF];
+};
+
+// Phi with its six ghost faces (x-, x+, y-, y+, z-, z+).  Face arrays are indexed
+// [j + ny*k], [i + nx*k], [i + nx*j].
+struct Phi {
+    const double* c;
+    const double* gx0; const double* gx1;
+    const double* gy0; const double* gy1;
+    const double* gz0; const double* gz1;
+};
+
+void set_error(const char* fmt, ...);
+
+// Kernels (and cuFFT executions) that can be timed one by one with CUDA events.
+enum KernelId { K_EUL_GAS = 0, K_LAG_GAS, K_EUL_BME, K_LAG_BME, K_CFL, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV,
+                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_NUM };
+
+struct Timing {
+    bool on = false;
+    cudaEvent_t* ev = nullptr;   // pairs: ev[2*i] start, ev[2*i+1] stop
+    int* kid = nullptr;
+    size_t cap = 0, used = 0;
+    double ms[K_NUM] = {};
+    long long cnt[K_NUM] = {};
+};
+
+}  // namespace gp
+
+struct gp_ctx {
+    gp_grid g;
+    double gamma;
+    gp_bc bc;
+    cudaStream_t stream;
+    size_t N;
+
+    // storage
+    char* base;
+    size_t bytes;
+    bool owns;
+    bool ready;
+    double* U[gp::NHYD];    // state U^n (and U^{n+1} after a step)
+    double* Us[gp::NHYD];   // U* between the stages
+    double* W[3];           // post-Eulerian velocity w* of the component in flight
+    double* phi;
+    double* phig[6];
+    double* d_dt;                   // [0] = dt of the last gp_max_dt
+    unsigned long long* d_smax;     // bit pattern of the running max signal speed
+    int* d_flag;                    // != 0: bad state seen by the CFL reduction
+
+    // Poisson
+    bool fft_ready;
+    cufftHandle plan_fwd, plan_inv;
+    cufftDoubleComplex* spec;       // half-spectrum work array
+    double* padded;                 // isolated: (2nx)(2ny)(2nz) real array
+    double* kspec;                  // isolated: real spectrum of the 1/r kernel
+    double* tabx; double* taby; double* tabz;   // periodic: 1 - (2/3) sin^2(pi k/N) per axis
+
+    long long n_own, n_fft;
+    gp::Timing* tim;
+};
+
+namespace gp {
+
+// api.cu: bracket one launch with events when timing is on
+void tic(gp_ctx* c, int kid);
+void toc(gp_ctx* c);
+
+// hydro.cu
+int launch_eulerian_gas(gp_ctx* c, double dt, const double* d_dt);
+int launch_eulerian_bme(gp_ctx* c, double dt, const double* d_dt);
+int launch_lagrangian(gp_ctx* c, int f0, int nf, double dt, const double* d_dt);
+int launch_cfl(gp_ctx* c, double cfl);
+int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz);
+
+// poisson.cu
+int poisson_setup(gp_ctx* c);
+void poisson_teardown(gp_ctx* c);
+int poisson_solve(gp_ctx* c);
+size_t poisson_storage_bytes(const gp_grid* g);
+
+}  // namespace gp
+
+#define GP_CUDA(call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            gp::set_error("%s:%d: %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return GP_ERR_CUDA;                                                                \
+        }                                                                                      \
+    } while (0)
+
+#define GP_CUFFT(call)                                                             \
+    do {                                                                           \
+        cufftResult r_ = (call);                                                   \
+        if (r_ != CUFFT_SUCCESS) {                                                 \
+            gp::set_error("%s:%d: %s: cufft error %d", __FILE__, __LINE__, #call, (int)r_); \
+            return GP_ERR_CUFFT;                                                   \
+        }                                                                          \
+    } while (0)

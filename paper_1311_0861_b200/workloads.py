@@ -254,12 +254,8 @@ def _disks(name, n, disks, steps, cfl, poisson, gamma, rd_cells, zd_cells, gas_f
         phiz = ax[0] * ey - ax[1] * ex
         return prof, R, (phix, phiy, phiz)
 
-    norms = []
-    for d in disks:
-        tot = 0.0
-        for z0 in range(0, n, 16):
-            tot += float(geometry(d, z0, min(n, z0 + 16))[0].sum())
-        norms.append(d.mass / (tot * h ** 3))
+    # analytic normalisation of the untruncated double-exponential profile: M = 4 pi A rd^2 zd
+    norms = [d.mass / (4.0 * np.pi * rd * rd * zd) for d in disks]
 
     def gen(z0, z1):
         shape = (z1 - z0, n, n)

@@ -1,0 +1,57 @@
+"""CPU-side checks of the boundary: the C-ABI library loads and exports every symbol that
+include/gpupegas.h declares (no compute calls without a GPU), and it fails loudly, not silently,
+when no CUDA device is present."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "gpupegas.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gp_[a-z_]+)\s*\(", text)))
+
+
+def test_header_declares_the_boundary_calls():
+    syms = declared_symbols()
+    for s in ("gp_create", "gp_set_state", "gp_step", "gp_solve_poisson", "gp_max_dt", "gp_get_state", "gp_destroy"):
+        assert s in syms
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_1311_0861_b200 import binding, build
+    build.build()
+    L = binding.lib()
+    for s in declared_symbols():
+        assert hasattr(L, s), s
+    assert sorted(binding.EXPORTS) == declared_symbols()
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    import paper_1311_0861_b200 as pkg
+    with pytest.raises(RuntimeError):
+        pkg.Simulation(8, 8, 8, 0.1)
+    # and straight through the C ABI
+    L = pkg.lib()
+    g = pkg.binding.gp_grid(8, 8, 8, 0.1, 1, 0, 1.0)
+    b = pkg.binding.gp_bc(0, 0, 0)
+    assert not L.gp_create(ctypes.byref(g), 1.4, ctypes.byref(b))
+    assert b"no CUDA device" in L.gp_last_error()
+
+
+def test_product_path_does_not_touch_the_oracle():
+    """Nothing under paper_1311_0861_b200/ or bench.py's product arm may import oracle/."""
+    pkg_dir = os.path.join(ROOT, "paper_1311_0861_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "liboracle" not in text and "oracle.h" not in text, f
