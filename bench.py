@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py — cell-updates/s per full timestep (fp64) of the GPUPEGAS hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 512] [--poisson periodic|isolated]
+
+A "step" is one pass of the whole hot path over the synthetic workload: gp_max_dt (device-resident
+dt) + gp_solve_poisson + gp_step.  Default workload = BASELINE.json config 5 (two-galaxy collision,
+512^3, gas + collisionless component + periodic FFT gravity).  Prints ONE JSON line on rank 0.
+
+  value      device-resident throughput, CUDA events on the library's stream, max over ranks
+  e2e        same metric through the C ABI with pinned HOST buffers: every step copies the 15
+             state fields host->device, runs the full timestep, and copies them back
+  roofline   dominant own kernel: algorithmic bytes per launch / its mean CUDA-event duration,
+             measured in the same timed region (gp_timing_*), against MEASURED_PEAKS.json
+  cpu_baseline  the CPU oracle as it stands, timed on the host cores on a bounded sample
+
+--impl reference times the CPU oracle (this tier's reference arm) on a bounded sample of the
+same workload; it is the only other place this file executes oracle/.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/s per full timestep (fp64)"
+UNIT = "cell-updates/s"
+W = 8  # bytes per fp64 word
+
+# Algorithmic bytes per cell of each own kernel: every array the stage
+# must read or write crosses HBM once (SURVEY.md 8(a) in->out column, 8(d) for the fused forms).
+ALGO_BYTES_PER_CELL = {
+    "eulerian_gas": (5 + 1 + 4) * W,        # a-2: reads 5 fields + Phi, writes 4 (rho* = rho)
+    "lagrangian_gas": (5 + 5) * W,          # a-3
+    "eulerian_bme": (10 + 1 + 9) * W,       # a-4
+    "lagrangian_bme": (10 + 10) * W,        # a-5
+    "hydro_gas_fused": (5 + 1 + 5) * W,     # 8(d): R5 + RPhi + W5
+    "hydro_bme_fused": (10 + 1 + 10) * W,   # 8(d): R10 + RPhi + W10
+    "cfl": 15 * W,                          # a-6
+    "poisson_source": 3 * W,
+    "poisson_green": 2 * W,                 # half spectrum, complex: read + write (nx/2+1)/nx * 16 B each
+}
+# minimum bytes per cell per FULL step for the headline roofline fraction
+STEP_BYTES_PER_CELL = {("gas",): 80, ("gas", "isolated"): 304, ("gas", "stars", "periodic"): 336,
+                       ("gas", "stars", "isolated"): 472}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def stored_traffic(kernel, workload_key):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture, or None."""
+    path = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        d = json.load(open(path))
+        return d.get(workload_key, {}).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, uuid, period=0.02):
+        super().__init__(daemon=True)
+        self.uuid, self.period = uuid, period
+        self.sm, self.reasons, self.sm_max, self.power = [], set(), None, []
+        self._stop_evt = threading.Event()
+        self.error = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            try:
+                h = nv.nvmlDeviceGetHandleByUUID(self.uuid.encode())
+            except Exception:
+                h = nv.nvmlDeviceGetHandleByUUID(self.uuid)
+            self.sm_max = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+                getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+                getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+                getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            }
+            get = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+            while not self._stop_evt.is_set():
+                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                except Exception:
+                    pass
+                r = get(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                time.sleep(self.period)
+        except Exception as e:  # NVML missing: report it, do not fake a clock
+            self.error = repr(e)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        out = {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons), "samples": len(self.sm)}
+        if self.sm:
+            s = sorted(self.sm)
+            out["sm_mhz"] = s[len(s) // 2]
+        if self.power:
+            out["power_w_max"] = max(self.power)
+        if self.error:
+            out["error"] = self.error
+        return out
+
+
+def make_workload(args):
+    from paper_1311_0861_b200 import workloads as wl
+    poisson = wl.POISSON_PERIODIC if args.poisson == "periodic" else wl.POISSON_ISOLATED
+    w = wl.two_disks(n=args.n, poisson=poisson)
+    name = f"two_disks_{args.n}^3 (BASELINE.json config 5: gas + collisionless + {args.poisson} FFT gravity)"
+    return w, name
+
+
+def oracle_leg(sample_n, poisson, max_steps, budget_s):
+    """Time the CPU oracle, as it stands, on a bounded sample of the workload (same recipe at
+    sample_n^3, same cells per disk scale).  Returns (cells/s, threads, description, ms/step)."""
+    import oracle
+    from paper_1311_0861_b200 import workloads as wl
+    w = wl.two_disks(n=sample_n, poisson=wl.POISSON_PERIODIC if poisson == "periodic" else wl.POISSON_ISOLATED)
+    o = oracle.Oracle(w.nx, w.ny, w.nz, w.h, w.components, w.poisson, w.G, w.gamma, w.bc)
+    o.set_state(w.state())
+    threads = oracle.get_threads()
+
+    def step():
+        o.solve_poisson()
+        o.step(o.max_dt(w.cfl))
+
+    step()  # warm-up (page faults, kernel spectrum)
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_steps and (n == 0 or time.perf_counter() - t0 < budget_s):
+        step()
+        n += 1
+    dt = time.perf_counter() - t0
+    desc = (f"{n} full steps (max_dt + {poisson} Poisson + step) of the two_disks recipe at {sample_n}^3 "
+            f"({w.cells} cells), OpenMP on outer loops, {threads} threads")
+    return w.cells * n / dt, threads, desc, 1e3 * dt / n
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    _, wname = make_workload_name_only(args)
+    # each "step" is a bounded sample: one full oracle step at sample_n^3
+    import oracle
+    from paper_1311_0861_b200 import workloads as wl
+    sample_n = args.ref_n
+    w = wl.two_disks(n=sample_n, poisson=wl.POISSON_PERIODIC if args.poisson == "periodic" else wl.POISSON_ISOLATED)
+    o = oracle.Oracle(w.nx, w.ny, w.nz, w.h, w.components, w.poisson, w.G, w.gamma, w.bc)
+    o.set_state(w.state())
+
+    def step():
+        o.solve_poisson()
+        o.step(o.max_dt(w.cfl))
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    value = w.cells * args.steps / dt
+    threads = oracle.get_threads()
+    sample = (f"each step = one full oracle step of the same recipe at {sample_n}^3 ({w.cells} cells); "
+              f"{args.steps} steps timed with perf_counter")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wname, "reference": "CPU oracle (oracle/, plain C++17) on host cores", "sample_grid": [sample_n] * 3},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def make_workload_name_only(args):
+    return None, f"two_disks_{args.n}^3 (BASELINE.json config 5: gas + collisionless + {args.poisson} FFT gravity)"
+
+
+def run_gpu(args):
+    import numpy as np
+    import torch
+    import paper_1311_0861_b200 as pkg
+    from paper_1311_0861_b200 import distrib
+
+    rank, local_rank, world = distrib.env_world()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    distrib.init("nccl", dev)
+    pkg.lib()
+
+    w, wname = make_workload(args)
+    names = w.field_names
+    cells = w.cells
+    t_setup = time.perf_counter()
+    # inputs: generated on the host (seeded, synthetic) into pinned buffers, handed over through the C ABI
+    host = {k: torch.empty((w.nz, w.ny, w.nx), dtype=torch.float64, pin_memory=True) for k in names}
+    w.fill({k: v.numpy() for k, v in host.items()})
+    sim = pkg.Simulation.from_workload(w)
+    for k in names:
+        sim.set(k, host[k].numpy())
+    sim.synchronize()
+    t_setup = time.perf_counter() - t_setup
+
+    def full_step():
+        sim.max_dt(w.cfl, to_host=False)
+        sim.solve_poisson()
+        sim.step(0.0)
+
+    for _ in range(args.warmup):
+        full_step()
+    sim.synchronize()
+    own0, fft0 = sim.launch_counts()
+
+    uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid).replace("GPU-", "")
+    sampler = ClockSampler(uuid)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.timing(True)
+    distrib.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0.record()
+    for _ in range(args.steps):
+        full_step()
+    ev1.record()
+    torch.cuda.synchronize()
+    distrib.barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    kernels = sim.timing_read()
+    sim.timing(False)
+    own1, fft1 = sim.launch_counts()
+    ms_max = distrib.max_over_ranks(ms, dev)
+    value = distrib.aggregate_throughput(cells, args.steps, ms_max, world)
+
+    # the state must still be physical after the timed steps (no work skipped, no blow-up)
+    dt_end = sim.max_dt(w.cfl)
+
+    # ---- end to end through the C ABI with host buffers --------------------------------------
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+    out = {k: torch.empty((w.nz, w.ny, w.nx), dtype=torch.float64, pin_memory=True) for k in names}
+
+    def e2e_step():
+        for k in names:
+            sim.set(k, host[k].numpy())            # H2D inside the timed region
+        sim.max_dt(w.cfl)                          # dt comes back to the host
+        sim.solve_poisson()
+        sim.step(0.0)
+        for k in names:
+            sim.get(k, out=out[k].numpy())         # D2H of the step's result
+
+    e2e_step()
+    distrib.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_ms_max = distrib.max_over_ranks(1e3 * e2e_s, dev)
+    e2e_value = distrib.aggregate_throughput(cells, e2e_steps, e2e_ms_max, world)
+    bytes_dir = len(names) * cells * W
+
+    if rank != 0:
+        distrib.shutdown()
+        return
+
+    # ---- roofline of the dominant own kernel ---------------------------------------------------
+    peak, peak_src = measured_peak()
+    own = {k: v for k, v in kernels.items() if not k.startswith("cufft")}
+    top = max(own, key=lambda k: own[k][0])
+    top_ms = own[top][0] / own[top][1]
+    algo = ALGO_BYTES_PER_CELL.get(top, 0) * cells
+    achieved = algo / (top_ms * 1e-3) / 1e9
+    wkey = f"two_disks_{args.n}_{args.poisson}"
+    roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": stored_traffic(top, wkey), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": algo, "ms_per_launch": top_ms}
+    step_bytes = STEP_BYTES_PER_CELL[("gas", "stars", args.poisson)]
+    per_gpu = value / world
+    step_roofline = {"bytes_per_cell_step": step_bytes,
+                     "frac_of_8TBs": per_gpu * step_bytes / 8.0e12,
+                     "frac_of_measured": per_gpu * step_bytes / (peak * 1e9)}
+    breakdown = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps} for k, v in kernels.items()}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, threads, desc, _ = oracle_leg(args.ref_n, args.poisson, max_steps=20, budget_s=12.0)
+        cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wname, "grid": [w.nx, w.ny, w.nz], "components": "gas+stars", "poisson": args.poisson,
+                   "cfl": w.cfl, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                   "cache": f"inputs larger than L2: {len(names) * cells * W / 1e9:.1f} GB of state per step vs 126 MB L2 (no flush)",
+                   "dt_after_run": dt_end, "setup_s": round(t_setup, 1)},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": bytes_dir, "d2h_bytes_per_step": bytes_dir,
+                "steps": e2e_steps, "ms_per_step": e2e_ms_max / e2e_steps},
+        "gpu_launches": int(own1 - own0), "cufft_execs": int(fft1 - fft0),
+        "roofline": roofline, "step_roofline": step_roofline, "kernels": breakdown,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    distrib.shutdown()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=512, help="grid size of the two-disk workload (BASELINE config 5: 512)")
+    ap.add_argument("--poisson", default="periodic", choices=["periodic", "isolated"])
+    ap.add_argument("--ref-n", type=int, default=128, help="grid size of the bounded sample the CPU oracle is timed on")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3          # timing hygiene: at least three warm-up steps
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -56,6 +56,22 @@ class Workload:
     def state(self):
         return self.fields(0, self.nz)
 
+    def fill(self, out, slab=8, threads=None):
+        """Generate the state slab by slab (in a thread pool) into preallocated arrays
+        out[name] of shape (nz, ny, nx), e.g. views of pinned host tensors."""
+        import os
+        from concurrent.futures import ThreadPoolExecutor
+
+        def work(z0):
+            z1 = min(self.nz, z0 + slab)
+            for k, v in self.fields(z0, z1).items():
+                out[k][z0:z1] = v
+
+        threads = threads or min(32, os.cpu_count() or 1)
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            list(ex.map(work, range(0, self.nz, slab)))
+        return out
+
 
 def _centres(n, h, lo=0, hi=None):
     hi = n if hi is None else hi
