@@ -18,6 +18,7 @@
  *     stream; see gp_set_stream).  Calls that hand a result to the host (gp_get_state to a
  *     host pointer, gp_max_dt with dt != NULL) synchronise that stream.
  *   - Cubic cells only (one h).  nx, ny, nz >= 4.  With a Poisson mode, nx, ny, nz even.
+ *     GP_POISSON_ISOLATED needs GP_BC_OUTFLOW on every axis (gp_create fails otherwise).
  *   - One "full timestep" of the metric = gp_max_dt + gp_solve_poisson (if gravity) + gp_step.
  */
 #ifndef GPUPEGAS_H
@@ -108,6 +109,14 @@ int gp_launch_counts(gp_ctx* ctx, long long* own_kernels, long long* cufft_execs
 int gp_timing_enable(gp_ctx* ctx, int on);
 int gp_timing_read(gp_ctx* ctx, int max_entries, int* n_entries, const char** names, double* total_ms,
                    long long* launches);
+
+/* ---- optional: self test of the device arithmetic helpers ----
+ * The hydro kernels replace fp64 divisions and square roots by a reciprocal and a reciprocal
+ * square root built from the hardware seed plus one cubically convergent correction.  This call
+ * evaluates both on n host-supplied positive normal numbers x (host pointers, n >= 1) so a test
+ * can bound their error: rcp[i] ~ 1/x[i], rsqrt_out[i] ~ 1/sqrt(x[i]).  Allocates and frees its
+ * own scratch; uses the default stream; synchronises. */
+int gp_math_selftest(int n, const double* x, double* rcp, double* rsqrt_out);
 
 #ifdef __cplusplus
 }

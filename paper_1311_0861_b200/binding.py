@@ -22,7 +22,7 @@ GAS_FIELDS, STAR_FIELDS = FIELDS[:5], FIELDS[5:15]
 # the symbols include/gpupegas.h declares
 EXPORTS = ["gp_create", "gp_destroy", "gp_set_state", "gp_get_state", "gp_solve_poisson", "gp_max_dt",
            "gp_step", "gp_last_error", "gp_set_stream", "gp_storage_bytes", "gp_bind_storage",
-           "gp_synchronize", "gp_launch_counts", "gp_timing_enable", "gp_timing_read"]
+           "gp_synchronize", "gp_launch_counts", "gp_timing_enable", "gp_timing_read", "gp_math_selftest"]
 
 
 class gp_grid(C.Structure):
@@ -70,8 +70,18 @@ def lib():
         L.gp_launch_counts.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
         L.gp_timing_enable.argtypes = [vp, C.c_int]
         L.gp_timing_read.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_char_p), dp, C.POINTER(C.c_longlong)]
+        L.gp_math_selftest.argtypes = [C.c_int, vp, vp, vp]
         _lib = L
     return _lib
+
+
+def math_selftest(x):
+    """(1/x, 1/sqrt(x)) as the hydro kernels compute them, for a numpy float64 array x > 0."""
+    import numpy as np
+    x = np.ascontiguousarray(x, dtype=np.float64).ravel()
+    r, s = np.empty_like(x), np.empty_like(x)
+    _chk(lib().gp_math_selftest(x.size, x.ctypes.data, r.ctypes.data, s.ctypes.data), "gp_math_selftest")
+    return r, s
 
 
 def _chk(code, what):

@@ -21,7 +21,8 @@ static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 static const char* const kKernelNames[K_NUM] = {
     "eulerian_gas", "lagrangian_gas", "eulerian_bme", "lagrangian_bme", "cfl", "poisson_source", "cufft_forward",
-    "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract"};
+    "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract",
+    "hydro_gas_fused", "hydro_bme_fused"};
 
 void tic(gp_ctx* c, int kid) {
     Timing* t = c->tim;
@@ -77,7 +78,7 @@ static size_t storage_bytes(const gp_grid& g) {
     size_t nf = 0;
     if (g.components & GP_GAS) nf += NGAS;
     if (g.components & GP_STARS) nf += NBME;
-    size_t b = (2 * nf + 3 + 1) * fb;                 // U, U*, w*, Phi
+    size_t b = (2 * nf + 1) * fb;                     // U, the step's target, Phi
     b += 6 * align256(ghost_elems(g) / 2 * sizeof(double));   // generous: each face <= half of the total
     b += 256;                                         // dt, smax, flag
     b += poisson_storage_bytes(&g);
@@ -113,7 +114,6 @@ static int ensure_storage(gp_ctx* c) {
             c->Us[f] = (double*)take(N * sizeof(double));
         }
     }
-    for (int d = 0; d < 3; ++d) c->W[d] = (double*)take(N * sizeof(double));
     c->phi = (double*)take(N * sizeof(double));
     const size_t face[3] = {(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny};
     for (int s = 0; s < 6; ++s) c->phig[s] = (double*)take(face[s / 2] * sizeof(double));
@@ -121,6 +121,9 @@ static int ensure_storage(gp_ctx* c) {
     c->d_dt = (double*)small;
     c->d_smax = (unsigned long long*)(small + 64);
     c->d_flag = (int*)(small + 128);
+    c->d_smax_next = (unsigned long long*)(small + 160);
+    c->d_flag_next = (int*)(small + 192);
+    c->cfl_cached = false;
     c->spec = nullptr; c->padded = nullptr; c->kspec = nullptr; c->tabx = c->taby = c->tabz = nullptr;
     if (g.poisson == GP_POISSON_PERIODIC) {
         c->spec = (cufftDoubleComplex*)take(((size_t)g.nx / 2 + 1) * g.ny * g.nz * sizeof(cufftDoubleComplex));
@@ -169,6 +172,10 @@ gp_ctx* gp_create(const gp_grid* grid, double gamma, const gp_bc* bc) {
     const int b[3] = {bc->x, bc->y, bc->z};
     for (int d = 0; d < 3; ++d)
         if (b[d] != GP_BC_PERIODIC && b[d] != GP_BC_OUTFLOW) { set_error("gp_create: bad boundary code"); return nullptr; }
+    if (grid->poisson == GP_POISSON_ISOLATED && (b[0] != GP_BC_OUTFLOW || b[1] != GP_BC_OUTFLOW || b[2] != GP_BC_OUTFLOW)) {
+        set_error("gp_create: the isolated Poisson mode needs outflow hydro boundaries on every axis");
+        return nullptr;
+    }
     if (!(gamma > 1.0)) { set_error("gp_create: gamma must exceed 1"); return nullptr; }
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -278,6 +285,7 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));   // the host buffer may be reused on return
     if (field == GP_PHI) return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
+    c->cfl_cached = false;
     return GP_OK;
 }
 
@@ -304,7 +312,8 @@ int gp_max_dt(gp_ctx* c, double cfl, double* dt) {
     if (!c || !(cfl > 0.0)) { set_error("gp_max_dt: bad argument"); return GP_ERR_ARG; }
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
-    rc = launch_cfl(c, cfl);
+    // after a step the fused kernels have already folded the max signal speed of the new state
+    rc = c->cfl_cached ? launch_cfl_from_cache(c, cfl) : launch_cfl(c, cfl);
     if (rc != GP_OK) return rc;
     if (dt) {
         double h_dt = 0.0;
@@ -324,15 +333,22 @@ int gp_step(gp_ctx* c, double dt) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     const double* d_dt = dt > 0.0 ? nullptr : c->d_dt;
+    if ((rc = launch_cfl_reset_next(c)) != GP_OK) return rc;
     if (c->g.components & GP_GAS) {
-        if ((rc = launch_eulerian_gas(c, dt, d_dt)) != GP_OK) return rc;
-        if ((rc = launch_lagrangian(c, 0, NGAS, dt, d_dt)) != GP_OK) return rc;
+        if ((rc = launch_fused_gas(c, dt, d_dt)) != GP_OK) return rc;
+        for (int f = 0; f < NGAS; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
     }
     if (c->g.components & GP_STARS) {
-        if ((rc = launch_eulerian_bme(c, dt, d_dt)) != GP_OK) return rc;
-        if ((rc = launch_lagrangian(c, NGAS, NBME, dt, d_dt)) != GP_OK) return rc;
+        if ((rc = launch_fused_bme(c, dt, d_dt)) != GP_OK) return rc;
+        for (int f = NGAS; f < NHYD; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
     }
+    c->cfl_cached = true;
     return GP_OK;
+}
+
+int gp_math_selftest(int n, const double* x, double* rcp, double* rsqrt_out) {
+    if (n < 1 || !x || !rcp || !rsqrt_out) { set_error("gp_math_selftest: bad argument"); return GP_ERR_ARG; }
+    return math_selftest(n, x, rcp, rsqrt_out);
 }
 
 }  // extern "C"

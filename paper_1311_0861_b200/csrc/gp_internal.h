@@ -45,7 +45,7 @@ void set_error(const char* fmt, ...);
 
 // Kernels (and cuFFT executions) that can be timed one by one with CUDA events.
 enum KernelId { K_EUL_GAS = 0, K_LAG_GAS, K_EUL_BME, K_LAG_BME, K_CFL, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV,
-                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_NUM };
+                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_FUSED_GAS, K_FUSED_BME, K_NUM };
 
 struct Timing {
     bool on = false;
@@ -70,14 +70,16 @@ struct gp_ctx {
     size_t bytes;
     bool owns;
     bool ready;
-    double* U[gp::NHYD];    // state U^n (and U^{n+1} after a step)
-    double* Us[gp::NHYD];   // U* between the stages
-    double* W[3];           // post-Eulerian velocity w* of the component in flight
+    double* U[gp::NHYD];    // state U^n
+    double* Us[gp::NHYD];   // target of the fused step (U^{n+1}); swapped with U after every step
     double* phi;
     double* phig[6];
     double* d_dt;                   // [0] = dt of the last gp_max_dt
     unsigned long long* d_smax;     // bit pattern of the running max signal speed
     int* d_flag;                    // != 0: bad state seen by the CFL reduction
+    unsigned long long* d_smax_next;   // max signal speed of U^{n+1}, folded by the fused step kernels
+    int* d_flag_next;
+    bool cfl_cached;                // d_smax_next / d_flag_next describe the current state
 
     // Poisson
     bool fft_ready;
@@ -98,11 +100,15 @@ void tic(gp_ctx* c, int kid);
 void toc(gp_ctx* c);
 
 // hydro.cu
-int launch_eulerian_gas(gp_ctx* c, double dt, const double* d_dt);
-int launch_eulerian_bme(gp_ctx* c, double dt, const double* d_dt);
-int launch_lagrangian(gp_ctx* c, int f0, int nf, double dt, const double* d_dt);
 int launch_cfl(gp_ctx* c, double cfl);
+int launch_cfl_from_cache(gp_ctx* c, double cfl);
+int launch_cfl_reset_next(gp_ctx* c);
 int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz);
+
+// fused.cu
+int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt);
+int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt);
+int math_selftest(int n, const double* x, double* rcp, double* rsq);
 
 // poisson.cu
 int poisson_setup(gp_ctx* c);

@@ -239,3 +239,16 @@ def test_poisson_non_power_of_two_against_stencil(pkg, orc):
     res = 6.0 * (a - phi) / (h * h) - 4 * np.pi * G * (rho - rho.mean())
     assert np.abs(res).max() < 1e-11 * 4 * np.pi * G * rho.max()
     assert abs(phi.mean()) < 1e-12 * np.abs(phi).max()
+
+
+def test_device_reciprocal_and_rsqrt_are_accurate_to_a_few_ulp(pkg):
+    """The hydro kernels use 1/x and 1/sqrt(x) built from the hardware seed plus one cubic
+    correction; bound their error over 60 decades against numpy's correctly rounded results."""
+    rng = np.random.default_rng(11)
+    x = np.concatenate([10.0 ** rng.uniform(-30, 30, 200000), rng.uniform(0.5, 2.0, 200000),
+                        np.array([1.0, 2.0, 4.0, 0.25, 3.0, 1e-4, 1e4])])
+    r, s = pkg.math_selftest(x)
+    ulp = np.finfo(np.float64).eps
+    assert np.abs(r * x - 1.0).max() <= 4 * ulp
+    exact = 1.0 / np.sqrt(x)
+    assert (np.abs(s - exact) / exact).max() <= 4 * ulp
