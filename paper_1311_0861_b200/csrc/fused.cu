@@ -4,16 +4,17 @@
 //
 // 2.5-D streaming.  A block of FX x FY = 32 x 16 threads owns an xy footprint (28 x 12 output
 // cells plus a two-cell halo) and marches along z.  Per plane it
-//   A  loads U^n (register prefetch one plane ahead), recovers primitives, publishes them in
-//      shared memory for the x/y neighbours;
-//   B  computes each x-, y- and z-face ONCE (hi face per thread; the lo face comes from the lane
-//      to the left by warp shuffle, from the row below through shared memory, from the previous
-//      plane in registers) and assembles U* of the footprint's inner ring;
-//   C  writes U* (density, velocity w* = momentum*/density, remaining fields) into a three-plane
-//      ring in shared memory -- U* never goes to HBM;
-//   D  advects plane k-1 of the ring: 4-vertex face velocities as separable (1/4,1/2,1/4)
+//   B  computes the x and y faces of plane j ONCE each (hi face per thread; the lo face comes
+//      from the lane to the left by warp shuffle and from the row below through shared memory);
+//   C  adds the flux differences and the gravity source to U*(j) held in registers;
+//   E  takes plane j+1 (staged asynchronously, cp.async, into the ring slot that is about to be
+//      rewritten), recovers its primitives, computes the z face (j, j+1), completes U*(j) and
+//      writes it (density, w* = momentum*/density, remaining fields) into a three-plane ring in
+//      shared memory -- U* never goes to HBM -- and publishes the primitives of plane j+1;
+//   D  advects plane j-1 of the ring: 4-vertex face velocities as separable (1/4,1/2,1/4)
 //      averages, upwind donor-cell fluxes in coefficient form, writes U^{n+1}, and folds the
 //      max signal speed of U^{n+1} into a block maximum.
+// Two block barriers per plane (after B, after E).
 // Ghost cells are index maps (wrap / clamp of the load address); for outflow the U* ghosts are
 // copies of the nearest interior U* (H6), restored in shared memory after step C.
 #include "gp_internal.h"
@@ -77,12 +78,13 @@ __device__ __forceinline__ PhiCol phi_col(const Geo& g, const Phi& P, int xv, in
     return c;
 }
 
-__device__ __forceinline__ double phi_load(const PhiCol& c, int kv, int zm, int nz) {
-    if (kv >= 0 && kv < nz) return c.p[(size_t)zm * c.stride];
-    if (c.zlo && kv == -1) return *c.zlo;
-    if (c.zlo && kv == nz) return *c.zhi;
-    return c.cm[(size_t)zm * c.nxny];
+__device__ __forceinline__ const double* phi_ptr(const PhiCol& c, int kv, int zm, int nz) {
+    if (kv >= 0 && kv < nz) return c.p + (size_t)zm * c.stride;
+    if (c.zlo && kv == -1) return c.zlo;
+    if (c.zlo && kv == nz) return c.zhi;
+    return c.cm + (size_t)zm * c.nxny;
 }
+__device__ __forceinline__ double phi_load(const PhiCol& c, int kv, int zm, int nz) { return *phi_ptr(c, kv, zm, nz); }
 
 // ---- face solvers ------------------------------------------------------------------------------
 // PAPER.md:112, 114 with Z = sqrt(rl rr gamma (pl+pr)/(rl+rr)) = num*r, 1/Z = den*r, r = rsqrt(num*den).
@@ -137,63 +139,101 @@ __device__ __forceinline__ void bme_face(double nl, const double ul[3], const do
     EF[5] = 2.0 * Ps[2] * us[2];
 }
 
-// ---- Lagrangian stage of one output cell from the U* ring ---------------------------------------
-// Ring slot layout: [field][PL], field 0 = density, 1..3 = w*, 4.. = the NO remaining fields.
-// Upwind flux form in coefficient form:
-//   F+ = max(w+,0) f0 + min(w+,0) f+,  F- = max(w-,0) f- + min(w-,0) f0
-//   f' = f0 - th (sum_d F+ - F-) = c0 f0 + sum_q c_q f_q
-// Momentum = density * w*, so its update is sum_q (c_q dens_q) w_q.
-template <int NO>
-__device__ __forceinline__ void lagrange_cell(const double* __restrict__ rm, const double* __restrict__ r0,
-                                              const double* __restrict__ rp, int t, double th,
-                                              double wxm, double wxp, double wym, double wyp, double wzm, double wzp,
-                                              double out[4 + NO]) {
-    const double cxm = th * fmax(wxm, 0.0), cxp = -th * fmin(wxp, 0.0);
-    const double cym = th * fmax(wym, 0.0), cyp = -th * fmin(wyp, 0.0);
-    const double czm = th * fmax(wzm, 0.0), czp = -th * fmin(wzp, 0.0);
-    const double sum = (fmax(wxp, 0.0) - fmin(wxm, 0.0)) + (fmax(wyp, 0.0) - fmin(wym, 0.0)) +
-                       (fmax(wzp, 0.0) - fmin(wzm, 0.0));
-    const double c0 = fma(-th, sum, 1.0);
-    // density-weighted coefficients
-    const double d0 = c0 * r0[t], dxm = cxm * r0[t - 1], dxp = cxp * r0[t + 1];
-    const double dym = cym * r0[t - FX], dyp = cyp * r0[t + FX];
-    const double dzm = czm * rm[t], dzp = czp * rp[t];
-    out[0] = ((d0 + dxm) + (dxp + dym)) + ((dyp + dzm) + dzp);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const double* w0 = r0 + (1 + d) * PL;
-        double v = d0 * w0[t];
-        v = fma(dxm, w0[t - 1], v);
-        v = fma(dxp, w0[t + 1], v);
-        v = fma(dym, w0[t - FX], v);
-        v = fma(dyp, w0[t + FX], v);
-        v = fma(dzm, rm[(1 + d) * PL + t], v);
-        v = fma(dzp, rp[(1 + d) * PL + t], v);
-        out[1 + d] = v;
-    }
-#pragma unroll
-    for (int f = 0; f < NO; ++f) {
-        const double* e0 = r0 + (4 + f) * PL;
-        double v = c0 * e0[t];
-        v = fma(cxm, e0[t - 1], v);
-        v = fma(cxp, e0[t + 1], v);
-        v = fma(cym, e0[t - FX], v);
-        v = fma(cyp, e0[t + FX], v);
-        v = fma(czm, rm[(4 + f) * PL + t], v);
-        v = fma(czp, rp[(4 + f) * PL + t], v);
-        out[4 + f] = v;
-    }
+// ---- shared-memory helpers ---------------------------------------------------------------------
+__device__ __forceinline__ double2 lds2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void sts2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+
+// 8-byte asynchronous global -> shared copy (LDGSTS): the next plane is staged without holding
+// registers while the current plane is computed.
+__device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
 }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // (1/4,1/2,1/4) average of three values
 __device__ __forceinline__ double avg3(double a, double b, double c) { return fma(0.25, a + c, 0.5 * b); }
 
-// 3x3 (omega x omega) average around t in a plane
-__device__ __forceinline__ double avg9(const double* __restrict__ s, int t) {
-    const double lo = avg3(s[t - FX - 1], s[t - FX], s[t - FX + 1]);
-    const double mi = avg3(s[t - 1], s[t], s[t + 1]);
-    const double hi = avg3(s[t + FX - 1], s[t + FX], s[t + FX + 1]);
+// Ring slot layout (doubles): pair plane P at offset P*2*PL, cell t at 2*t, two fields per cell:
+//   P0 = (density, w*_z)   P1 = (w*_x, w*_y)   P2.. = the remaining fields in pairs
+// so that every neighbour access is one 128-bit load.
+constexpr int PP = 2 * PL;   // doubles per pair plane
+
+// 3x3 (omega x omega) average of the second member of pair plane P0 (w*_z) around cell t
+__device__ __forceinline__ double avg9_wz(const double* __restrict__ r, int t) {
+    const double* s = r + 1;
+    const double lo = avg3(s[2 * (t - FX - 1)], s[2 * (t - FX)], s[2 * (t - FX + 1)]);
+    const double mi = avg3(s[2 * (t - 1)], s[2 * t], s[2 * (t + 1)]);
+    const double hi = avg3(s[2 * (t + FX - 1)], s[2 * (t + FX)], s[2 * (t + FX + 1)]);
     return avg3(lo, mi, hi);
+}
+
+// Upwind flux form of one cell in coefficient form:
+//   F+ = max(w+,0) f0 + min(w+,0) f+,  F- = max(w-,0) f- + min(w-,0) f0,
+//   f' = f0 - th (sum_d F+ - F-) = c0 f0 + sum_q c_q f_q,   max(w,0) = (w+|w|)/2, min(w,0) = (w-|w|)/2.
+struct LagCoef { double c0, xm, xp, ym, yp, zm, zp; };
+
+__device__ __forceinline__ LagCoef lag_coef(double th, double wxm, double wxp, double wym, double wyp, double wzm, double wzp) {
+    const double hth = 0.5 * th;
+    LagCoef c;
+    c.xm = hth * (wxm + fabs(wxm)); c.xp = hth * (fabs(wxp) - wxp);
+    c.ym = hth * (wym + fabs(wym)); c.yp = hth * (fabs(wyp) - wyp);
+    c.zm = hth * (wzm + fabs(wzm)); c.zp = hth * (fabs(wzp) - wzp);
+    const double sum = ((wxp + fabs(wxp)) + (fabs(wxm) - wxm)) + ((wyp + fabs(wyp)) + (fabs(wym) - wym)) +
+                       ((wzp + fabs(wzp)) + (fabs(wzm) - wzm));
+    c.c0 = fma(-hth, sum, 1.0);
+    return c;
+}
+
+// Lagrangian stage of one output cell from the U* ring.  Momentum = density * w*, so its update is
+// sum_q (c_q dens_q) w*_q.  out = (density, momentum x y z, NO remaining fields).
+template <int NO>
+__device__ __forceinline__ void lagrange_cell(const double* __restrict__ rm, const double* __restrict__ r0,
+                                              const double* __restrict__ rp, int t, const LagCoef& c, double out[4 + NO]) {
+    const double2 a0 = lds2(r0 + 2 * t), axm = lds2(r0 + 2 * (t - 1)), axp = lds2(r0 + 2 * (t + 1));
+    const double2 aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
+    const double2 azm = lds2(rm + 2 * t), azp = lds2(rp + 2 * t);
+    const double d0 = c.c0 * a0.x, dxm = c.xm * axm.x, dxp = c.xp * axp.x, dym = c.ym * aym.x, dyp = c.yp * ayp.x,
+                 dzm = c.zm * azm.x, dzp = c.zp * azp.x;
+    out[0] = ((d0 + dxm) + (dxp + dym)) + ((dyp + dzm) + dzp);
+    out[3] = fma(dzp, azp.y, fma(dzm, azm.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, d0 * a0.y))))));
+    {
+        const double2 b0 = lds2(r0 + PP + 2 * t), bxm = lds2(r0 + PP + 2 * (t - 1)), bxp = lds2(r0 + PP + 2 * (t + 1));
+        const double2 bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
+        const double2 bzm = lds2(rm + PP + 2 * t), bzp = lds2(rp + PP + 2 * t);
+        out[1] = fma(dzp, bzp.x, fma(dzm, bzm.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, d0 * b0.x))))));
+        out[2] = fma(dzp, bzp.y, fma(dzm, bzm.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, d0 * b0.y))))));
+    }
+#pragma unroll
+    for (int P = 0; P < (NO + 1) / 2; ++P) {
+        const int o = (2 + P) * PP;
+        if (2 * P + 1 < NO) {
+            const double2 e0 = lds2(r0 + o + 2 * t), exm = lds2(r0 + o + 2 * (t - 1)), exp_ = lds2(r0 + o + 2 * (t + 1));
+            const double2 eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
+            const double2 ezm = lds2(rm + o + 2 * t), ezp = lds2(rp + o + 2 * t);
+            out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.zm, ezm.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, c.c0 * e0.x))))));
+            out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.zm, ezm.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, c.c0 * e0.y))))));
+        } else {
+            const double e0 = r0[o + 2 * t], exm = r0[o + 2 * (t - 1)], exp_ = r0[o + 2 * (t + 1)];
+            const double eym = r0[o + 2 * (t - FX)], eyp = r0[o + 2 * (t + FX)];
+            const double ezm = rm[o + 2 * t], ezp = rp[o + 2 * t];
+            out[4 + 2 * P] = fma(c.zp, ezp, fma(c.zm, ezm, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, c.c0 * e0))))));
+        }
+    }
+}
+
+// Face velocities of one output cell (reading G2) from the z-averaged w*_x, w*_y pair plane
+// (s_tz) : x faces = mean of the y-averaged columns tx-1|tx and tx|tx+1, y faces likewise.
+__device__ __forceinline__ void face_vel_xy(const double* __restrict__ s_tz, int t, double& wxm, double& wxp, double& wym,
+                                            double& wyp) {
+    const double2 mm = lds2(s_tz + 2 * (t - FX - 1)), m0 = lds2(s_tz + 2 * (t - FX)), mp = lds2(s_tz + 2 * (t - FX + 1));
+    const double2 zm = lds2(s_tz + 2 * (t - 1)), z0 = lds2(s_tz + 2 * t), zp = lds2(s_tz + 2 * (t + 1));
+    const double2 pm = lds2(s_tz + 2 * (t + FX - 1)), p0 = lds2(s_tz + 2 * (t + FX)), pp = lds2(s_tz + 2 * (t + FX + 1));
+    const double a_m = avg3(mm.x, zm.x, pm.x), a_0 = avg3(m0.x, z0.x, p0.x), a_p = avg3(mp.x, zp.x, pp.x);
+    const double b_m = avg3(mm.y, m0.y, mp.y), b_0 = avg3(zm.y, z0.y, zp.y), b_p = avg3(pm.y, p0.y, pp.y);
+    wxm = 0.5 * (a_m + a_0); wxp = 0.5 * (a_0 + a_p);
+    wym = 0.5 * (b_m + b_0); wyp = 0.5 * (b_0 + b_p);
 }
 
 template <int NF>
@@ -275,393 +315,509 @@ __device__ __forceinline__ void block_max_commit(double smax, int bad, unsigned 
 }
 
 // =================================================================================================
-// Gas: fields rho, mx, my, mz, E.   Shared planes: 5 prims (rho, vx, vy, p, Phi), 2 y-flux,
-// 3 x 5 ring (rho, wx, wy, wz, E), 2 smoothing = 24 planes = 96 KB.
+// Gas: fields rho, mx, my, mz, E.
+// Shared planes (of PL doubles): (rho,p) pair 2, vx 1, vy 1, Phi 1, y-flux (P,PV) pair 2,
+// ring 3 x 3 pair planes = 18, z-averaged (w*_x,w*_y) pair 2  ->  27 planes = 108 KB.
+// The raw U of the next plane is staged (cp.async) in the ring slot that is about to be rewritten.
 // =================================================================================================
-constexpr int GAS_NR = 5;
-constexpr int GAS_PLANES = 5 + 2 + 3 * GAS_NR + 2;
+constexpr int GAS_SLOT = 3 * PP;
+constexpr int GAS_PLANES = 2 + 3 + 2 + 3 * 6 + 2;
+
+struct GasCarry {
+    double rho, ir, vx, vy, vz, p;        // primitives of the current plane j (own cell)
+    double amx, amy, amz, aE;             // U*(j) under construction
+    double phi0, phim;                    // Phi(j), Phi(j-1) of the own column
+    double Sz_prev, wzp_prev, smax;
+    int bad;
+};
+
+struct GasShared {
+    double *rp, *vx, *vy, *phi, *fy, *ring, *tz;
+};
+
+template <bool ST>
+__device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f, const PhiCol& pc, const GasShared& S,
+                                         GasCarry& c, int j, double tau, double th, double inv2h) {
+    const Geo& g = a.g;
+    const int t = f.t;
+    const double gamma = a.gamma, gm1 = a.gamma - 1.0;
+    const bool zout = g.bcz == GP_BC_OUTFLOW;
+    const bool top_copy = !ST && zout && j == g.nz;
+    const bool bot_dup = !ST && zout && j == 0;
+    const bool do_out = ST || j - 1 >= f.z0;
+    const bool do_wzp = ST || j >= f.z0;
+    const bool stage_next = ST || j + 1 <= f.z1;
+
+    // B: x and y faces of plane j (each computed once: hi face per thread)
+    double Pyh = 0.0, PVyh = 0.0, gy = 0.0;
+    if (f.ty <= FY - 2) {
+        const double2 r = lds2(S.rp + 2 * (t + FX));
+        gas_face(gamma, c.rho, c.vy, c.p, r.x, S.vy[t + FX], r.y, Pyh, PVyh);
+        sts2(S.fy + 2 * t, Pyh, PVyh);
+    }
+    if (f.star_row) {
+        const int tr = f.tx < FX - 1 ? t + 1 : t;
+        const double2 r = lds2(S.rp + 2 * tr);
+        double Pxh, PVxh;
+        gas_face(gamma, c.rho, c.vx, c.p, r.x, S.vx[tr], r.y, Pxh, PVxh);
+        const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1);
+        const double PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
+        const double gx = (S.phi[t + 1] - S.phi[t - 1]) * inv2h;
+        gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
+        const double trg = tau * c.rho * gx;
+        const double mx = c.rho * c.vx;
+        c.amx = c.amx - th * (Pxh - Pxl) - trg;
+        c.aE = c.aE - th * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
+    }
+    __syncthreads();
+
+    // C: y-flux difference
+    if (f.star_row) {
+        const double2 lo = lds2(S.fy + 2 * (t - FX));
+        const double trg = tau * c.rho * gy;
+        const double my = c.rho * c.vy;
+        c.amy = c.amy - th * (Pyh - lo.x) - trg;
+        c.aE = c.aE - th * (PVyh - lo.y) - fma(-0.5 * tau, trg, tau * my) * gy;
+    }
+
+    // E: plane j+1 arrives; z face (j, j+1); U*(j) complete -> ring slot j; publish primitives(j+1)
+    double* rs = S.ring + ring_slot(j) * GAS_SLOT;
+    cp_async_wait_all();
+    const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t), s2 = lds2(rs + 2 * PP + 2 * t);
+    const double rho_n = s0.x, mx_n = s0.y, my_n = s1.x, mz_n = s1.y, E_n = s2.x, phi_n = s2.y;
+    const double ir_n = frcp(rho_n);
+    const double vx_n = mx_n * ir_n, vy_n = my_n * ir_n, vz_n = mz_n * ir_n;
+    const double p_n = gm1 * (E_n - 0.5 * fma(mx_n, vx_n, fma(my_n, vy_n, mz_n * vz_n)));
+    double Pz = 0.0, PVz = 0.0;
+    if (f.star_row) {
+        gas_face(gamma, c.rho, c.vz, c.p, rho_n, vz_n, p_n, Pz, PVz);
+        double wx, wy, wz, Es, dens;
+        if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
+            const double* rq = S.ring + ring_slot(j - 1) * GAS_SLOT;
+            const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
+            dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y; Es = rq[2 * PP + 2 * t];
+        } else {
+            const double gz = (phi_n - c.phim) * inv2h;
+            const double trg = tau * c.rho * gz;
+            const double mz = c.rho * c.vz;
+            const double mzs = c.amz - th * Pz - trg;
+            Es = c.aE - th * PVz - fma(-0.5 * tau, trg, tau * mz) * gz;
+            dens = c.rho; wx = c.amx * c.ir; wy = c.amy * c.ir; wz = mzs * c.ir;
+        }
+        sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy); rs[2 * PP + 2 * t] = Es;
+        if (bot_dup) {                        // outflow: U*(-1) := U*(0)
+            double* rg = S.ring + ring_slot(-1) * GAS_SLOT;
+            sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy); rg[2 * PP + 2 * t] = Es;
+        }
+        if (do_out) {                         // z-average of w*_x, w*_y for plane j-1
+            const double2 wm = lds2(S.ring + ring_slot(j - 2) * GAS_SLOT + PP + 2 * t);
+            const double2 w0 = lds2(S.ring + ring_slot(j - 1) * GAS_SLOT + PP + 2 * t);
+            sts2(S.tz + 2 * t, avg3(wm.x, w0.x, wx), avg3(wm.y, w0.y, wy));
+        }
+    }
+    sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n; S.phi[t] = phi_n;
+    c.amx = mx_n; c.amy = my_n; c.amz = fma(th, Pz, mz_n); c.aE = fma(th, PVz, E_n);
+    c.rho = rho_n; c.ir = ir_n; c.vx = vx_n; c.vy = vy_n; c.vz = vz_n; c.p = p_n;
+    c.phim = c.phi0; c.phi0 = phi_n;
+    __syncthreads();
+
+    if (f.block_fix) {
+        if (f.fix) {
+#pragma unroll
+            for (int P = 0; P < 3; ++P) {
+                const double2 v = lds2(rs + P * PP + 2 * f.fix_src);
+                sts2(rs + P * PP + 2 * t, v.x, v.y);
+                if (bot_dup) sts2(S.ring + ring_slot(-1) * GAS_SLOT + P * PP + 2 * t, v.x, v.y);
+            }
+            const double2 v = lds2(S.tz + 2 * f.fix_src);
+            sts2(S.tz + 2 * t, v.x, v.y);
+        }
+        __syncthreads();
+    }
+
+    // D: Lagrangian stage of plane j-1 (ring planes j-2, j-1, j)
+    if (f.out_row) {
+        const double* rp = rs;
+        const double Sz_new = avg9_wz(rp, t);
+        if (bot_dup) c.Sz_prev = Sz_new;
+        if (do_wzp) {
+            const double wzp = 0.5 * (c.Sz_prev + Sz_new);
+            if (do_out) {
+                const double* r0 = S.ring + ring_slot(j - 1) * GAS_SLOT;
+                const double* rm = S.ring + ring_slot(j - 2) * GAS_SLOT;
+                double wxm, wxp, wym, wyp;
+                face_vel_xy(S.tz, t, wxm, wxp, wym, wyp);
+                const LagCoef lc = lag_coef(th, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
+                double out[NGAS];
+                lagrange_cell<1>(rm, r0, rp, t, lc, out);
+                if (f.is_out) {
+                    const size_t off = f.base + (size_t)(j - 1) * f.nxny;
+#pragma unroll
+                    for (int q = 0; q < NGAS; ++q) a.Un[q][off] = out[q];
+                    // CFL of the new state (reading G4)
+                    const double irn = frcp(out[0]);
+                    const double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
+                    const double pn = gm1 * (out[4] - 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz)));
+                    const double c2 = gamma * pn * irn;
+                    const double s = fmax(fmax(fabs(ux), fabs(uy)), fabs(uz)) + c2 * frsqrt(c2);
+                    if (!(out[0] > 0.0) || !(pn > 0.0) || !(s <= 1.7976931348623157e308)) c.bad = 1;
+                    c.smax = fmax(c.smax, s);
+                }
+            }
+            c.wzp_prev = wzp;
+        }
+        c.Sz_prev = Sz_new;
+    }
+    // stage plane j+2 into the slot D just finished with (own column only)
+    if (stage_next) {
+        const int zm = map_safe(j + 2, g.nz, g.bcz);
+        const size_t off = f.base + (size_t)zm * f.nxny;
+        double* st = S.ring + ring_slot(j + 1) * GAS_SLOT;
+        cp_async8(st + 2 * t, a.U[0] + off); cp_async8(st + 2 * t + 1, a.U[1] + off);
+        cp_async8(st + PP + 2 * t, a.U[2] + off); cp_async8(st + PP + 2 * t + 1, a.U[3] + off);
+        cp_async8(st + 2 * PP + 2 * t, a.U[4] + off);
+        cp_async8(st + 2 * PP + 2 * t + 1, phi_ptr(pc, j + 2, zm, g.nz));
+    }
+    cp_async_commit();
+}
 
 __global__ void __launch_bounds__(PL, 1)
 k_fused_gas(FusedArgs<NGAS> a) {
-    extern __shared__ double sm[];
-    double* s_rho = sm; double* s_vx = sm + PL; double* s_vy = sm + 2 * PL; double* s_p = sm + 3 * PL;
-    double* s_phi = sm + 4 * PL; double* s_fP = sm + 5 * PL; double* s_fPV = sm + 6 * PL;
-    double* ring = sm + 7 * PL;
-    double* s_tx = ring + 3 * GAS_NR * PL; double* s_ty = s_tx + PL;
+    extern __shared__ double2 sm2[];
+    double* sm = reinterpret_cast<double*>(sm2);
+    GasShared S;
+    S.rp = sm; S.vx = sm + 2 * PL; S.vy = sm + 3 * PL; S.phi = sm + 4 * PL; S.fy = sm + 5 * PL;
+    S.ring = sm + 7 * PL; S.tz = S.ring + 3 * GAS_SLOT;
 
-    const Geo g = a.g;
+    const Geo& g = a.g;
     const Foot f = make_foot(g, a.zchunk);
     const int t = f.t;
     const double tau = a.dt_ptr ? *a.dt_ptr : a.dt_val;
-    const double th = tau / a.h, inv2h = 0.5 / a.h, gamma = a.gamma, gm1 = a.gamma - 1.0;
+    const double th = tau / a.h, inv2h = 0.5 / a.h, gm1 = a.gamma - 1.0;
     const PhiCol pc = phi_col(g, a.phi, f.xv, f.yv, f.xm, f.ym);
-    const bool zout = g.bcz == GP_BC_OUTFLOW;
 
-    double nx_[NGAS], nphi;
-    {
-        const int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
-        const size_t off = f.base + (size_t)zm * f.nxny;
-#pragma unroll
-        for (int q = 0; q < NGAS; ++q) nx_[q] = a.U[q][off];
-        nphi = phi_load(pc, f.z0 - 2, zm, g.nz);
+    GasCarry c;
+    c.Sz_prev = c.wzp_prev = c.smax = 0.0; c.bad = 0;
+    {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
+        int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
+        size_t off = f.base + (size_t)zm * f.nxny;
+        double rho = a.U[0][off], mx = a.U[1][off], my = a.U[2][off], mz = a.U[3][off], E = a.U[4][off];
+        const double phi_a = phi_load(pc, f.z0 - 2, zm, g.nz);
+        double ir = frcp(rho);
+        const double vz_a = mz * ir;
+        const double p_a = gm1 * (E - 0.5 * ((mx * mx + my * my) * ir + mz * vz_a));
+        const double rho_a = rho;
+        zm = map_safe(f.z0 - 1, g.nz, g.bcz);
+        off = f.base + (size_t)zm * f.nxny;
+        rho = a.U[0][off]; mx = a.U[1][off]; my = a.U[2][off]; mz = a.U[3][off]; E = a.U[4][off];
+        const double phi_b = phi_load(pc, f.z0 - 1, zm, g.nz);
+        ir = frcp(rho);
+        c.rho = rho; c.ir = ir; c.vx = mx * ir; c.vy = my * ir; c.vz = mz * ir;
+        c.p = gm1 * (E - 0.5 * fma(mx, c.vx, fma(my, c.vy, mz * c.vz)));
+        double Pz, PVz;
+        gas_face(a.gamma, rho_a, vz_a, p_a, c.rho, c.vz, c.p, Pz, PVz);
+        c.amx = mx; c.amy = my; c.amz = fma(th, Pz, mz); c.aE = fma(th, PVz, E);
+        c.phim = phi_a; c.phi0 = phi_b;
+        sts2(S.rp + 2 * t, c.rho, c.p); S.vx[t] = c.vx; S.vy[t] = c.vy; S.phi[t] = phi_b;
+        // stage plane z0 where U*(z0-1) will be written
+        zm = map_safe(f.z0, g.nz, g.bcz);
+        off = f.base + (size_t)zm * f.nxny;
+        double* st = S.ring + ring_slot(f.z0 - 1) * GAS_SLOT;
+        cp_async8(st + 2 * t, a.U[0] + off); cp_async8(st + 2 * t + 1, a.U[1] + off);
+        cp_async8(st + PP + 2 * t, a.U[2] + off); cp_async8(st + PP + 2 * t + 1, a.U[3] + off);
+        cp_async8(st + 2 * PP + 2 * t, a.U[4] + off);
+        cp_async8(st + 2 * PP + 2 * t + 1, phi_ptr(pc, f.z0, zm, g.nz));
+        cp_async_commit();
     }
-    double pr_rho = 1.0, pr_ir = 1.0, pr_vz = 0.0, pr_mz = 0.0, pr_p = 1.0;
-    double acc_mx = 0.0, acc_my = 0.0, acc_mz = 0.0, acc_E = 0.0;
-    double phi_m1 = 0.0, phi_m2 = 0.0;
-    double Sz_prev = 0.0, wzp_prev = 0.0, smax = 0.0;
-    int bad = 0;
+    __syncthreads();
 
-    for (int kv = f.z0 - 2; kv <= f.z1 + 1; ++kv) {
-        const double rho = nx_[0], mx = nx_[1], my = nx_[2], mz = nx_[3], E = nx_[4], phi = nphi;
-        if (kv <= f.z1) {
-            const int zm = map_safe(kv + 1, g.nz, g.bcz);
-            const size_t off = f.base + (size_t)zm * f.nxny;
-#pragma unroll
-            for (int q = 0; q < NGAS; ++q) nx_[q] = a.U[q][off];
-            nphi = phi_load(pc, kv + 1, zm, g.nz);
-        }
-        // A: primitives (S0)
-        const double ir = frcp(rho);
-        const double vx = mx * ir, vy = my * ir, vz = mz * ir;
-        const double p = gm1 * (E - 0.5 * fma(mx, vx, fma(my, vy, mz * vz)));
-        s_rho[t] = rho; s_vx[t] = vx; s_vy[t] = vy; s_p[t] = p; s_phi[t] = phi;
-        __syncthreads();
-
-        // B: faces
-        const bool xy_stage = kv >= f.z0 - 1 && kv <= f.z1;
-        const bool z_stage = kv >= f.z0 - 1;
-        double Pyh = 0.0, PVyh = 0.0, Pxh = 0.0, PVxh = 0.0, Pxl = 0.0, PVxl = 0.0, Pz = 0.0, PVz = 0.0;
-        if (xy_stage && f.ty <= FY - 2) {
-            gas_face(gamma, rho, vy, p, s_rho[t + FX], s_vy[t + FX], s_p[t + FX], Pyh, PVyh);
-            s_fP[t] = Pyh; s_fPV[t] = PVyh;
-        }
-        if (f.star_row) {
-            if (xy_stage) {
-                const int tr = f.tx < FX - 1 ? t + 1 : t;
-                gas_face(gamma, rho, vx, p, s_rho[tr], s_vx[tr], s_p[tr], Pxh, PVxh);
-                Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1);
-                PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
-            }
-            if (z_stage) gas_face(gamma, pr_rho, pr_vz, pr_p, rho, vz, p, Pz, PVz);
-        }
-        __syncthreads();
-
-        // C: finish U*(kv-1), start U*(kv)
-        if (f.star_row) {
-            if (kv >= f.z0) {
-                double* rs = ring + ring_slot(kv - 1) * GAS_NR * PL;
-                if (zout && kv - 1 == g.nz) {          // top ghost plane := U*(nz-1)
-                    const double* rq = ring + ring_slot(kv - 2) * GAS_NR * PL;
-#pragma unroll
-                    for (int q = 0; q < GAS_NR; ++q) rs[q * PL + t] = rq[q * PL + t];
-                } else {
-                    const double gz = (phi - phi_m2) * inv2h;
-                    const double mzs = acc_mz - th * Pz - tau * pr_rho * gz;
-                    const double Es = acc_E - th * PVz - tau * (pr_mz - 0.5 * tau * pr_rho * gz) * gz;
-                    const double wx = acc_mx * pr_ir, wy = acc_my * pr_ir, wz = mzs * pr_ir;
-                    rs[t] = pr_rho; rs[PL + t] = wx; rs[2 * PL + t] = wy; rs[3 * PL + t] = wz; rs[4 * PL + t] = Es;
-                    if (zout && kv - 1 == 0) {         // bottom ghost plane := U*(0)
-                        double* rg = ring + ring_slot(-1) * GAS_NR * PL;
-                        rg[t] = pr_rho; rg[PL + t] = wx; rg[2 * PL + t] = wy; rg[3 * PL + t] = wz; rg[4 * PL + t] = Es;
-                    }
-                }
-            }
-            if (xy_stage) {
-                const double Pyl = s_fP[t - FX], PVyl = s_fPV[t - FX];
-                const double gx = (s_phi[t + 1] - s_phi[t - 1]) * inv2h;
-                const double gy = (s_phi[t + FX] - s_phi[t - FX]) * inv2h;
-                acc_mx = mx - th * (Pxh - Pxl) - tau * rho * gx;
-                acc_my = my - th * (Pyh - Pyl) - tau * rho * gy;
-                acc_mz = fma(th, Pz, mz);
-                acc_E = E - th * ((PVxh - PVxl) + (PVyh - PVyl)) + th * PVz -
-                        tau * ((mx - 0.5 * tau * rho * gx) * gx + (my - 0.5 * tau * rho * gy) * gy);
-            }
-        }
-        pr_rho = rho; pr_ir = ir; pr_vz = vz; pr_mz = mz; pr_p = p;
-        phi_m2 = phi_m1; phi_m1 = phi;
-        __syncthreads();
-
-        if (kv < f.z0) continue;
-        if (f.block_fix) {
-            if (f.fix) {
-                double* rs = ring + ring_slot(kv - 1) * GAS_NR * PL;
-#pragma unroll
-                for (int q = 0; q < GAS_NR; ++q) rs[q * PL + t] = rs[q * PL + f.fix_src];
-                if (zout && kv - 1 == 0) {
-                    double* rg = ring + ring_slot(-1) * GAS_NR * PL;
-#pragma unroll
-                    for (int q = 0; q < GAS_NR; ++q) rg[q * PL + t] = rg[q * PL + f.fix_src];
-                }
-            }
-            __syncthreads();
-        }
-
-        // D: Lagrangian stage of plane k = kv-2 (ring planes kv-3, kv-2, kv-1)
-        const double* rp = ring + ring_slot(kv - 1) * GAS_NR * PL;
-        const double* r0 = ring + ring_slot(kv - 2) * GAS_NR * PL;
-        const double* rm = ring + ring_slot(kv - 3) * GAS_NR * PL;
-        const bool do_out = kv >= f.z0 + 2;
-        if (do_out && f.star_row) {
-            s_tx[t] = avg3(rm[PL + t], r0[PL + t], rp[PL + t]);
-            s_ty[t] = avg3(rm[2 * PL + t], r0[2 * PL + t], rp[2 * PL + t]);
-        }
-        if (do_out) __syncthreads();
-        if (f.out_row) {
-            const double Sz_new = avg9(rp + 3 * PL, t);
-            if (zout && kv - 1 == 0) Sz_prev = Sz_new;
-            if (kv >= f.z0 + 1) {
-                const double wzp = 0.5 * (Sz_prev + Sz_new);
-                if (do_out) {
-                    const double a_m = avg3(s_tx[t - FX - 1], s_tx[t - 1], s_tx[t + FX - 1]);
-                    const double a_0 = avg3(s_tx[t - FX], s_tx[t], s_tx[t + FX]);
-                    const double a_p = avg3(s_tx[t - FX + 1], s_tx[t + 1], s_tx[t + FX + 1]);
-                    const double b_m = avg3(s_ty[t - FX - 1], s_ty[t - FX], s_ty[t - FX + 1]);
-                    const double b_0 = avg3(s_ty[t - 1], s_ty[t], s_ty[t + 1]);
-                    const double b_p = avg3(s_ty[t + FX - 1], s_ty[t + FX], s_ty[t + FX + 1]);
-                    double out[NGAS];
-                    lagrange_cell<1>(rm, r0, rp, t, th, 0.5 * (a_m + a_0), 0.5 * (a_0 + a_p), 0.5 * (b_m + b_0),
-                                     0.5 * (b_0 + b_p), wzp_prev, wzp, out);
-                    if (f.is_out) {
-                        const size_t off = f.base + (size_t)(kv - 2) * f.nxny;
-#pragma unroll
-                        for (int q = 0; q < NGAS; ++q) a.Un[q][off] = out[q];
-                        // CFL of the new state (reading G4)
-                        const double irn = frcp(out[0]);
-                        const double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
-                        const double pn = gm1 * (out[4] - 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz)));
-                        const double c2 = gamma * pn * irn;
-                        const double cs = c2 * frsqrt(c2);
-                        const double s = fmax(fmax(fabs(ux), fabs(uy)), fabs(uz)) + cs;
-                        if (!(out[0] > 0.0) || !(pn > 0.0) || !(s <= 1.7976931348623157e308)) bad = 1;
-                        smax = fmax(smax, s);
-                    }
-                }
-                wzp_prev = wzp;
-            }
-            Sz_prev = Sz_new;
-        }
-    }
-    block_max_commit(smax, bad, a.smax_bits, a.flag, s_rho);
+    int j = f.z0 - 1;
+    for (; j <= f.z0 && j <= f.z1; ++j) gas_iter<false>(a, f, pc, S, c, j, tau, th, inv2h);
+    for (; j <= f.z1 - 1; ++j) gas_iter<true>(a, f, pc, S, c, j, tau, th, inv2h);
+    for (; j <= f.z1; ++j) gas_iter<false>(a, f, pc, S, c, j, tau, th, inv2h);
+    cp_async_wait_all();
+    block_max_commit(c.smax, c.bad, a.smax_bits, a.flag, S.rp);
 }
 
 // =================================================================================================
-// Collisionless component: fields n, nu (3), nE_ij (6).  Shared planes: 10 prims (n, u3, Pixx,
-// Pixy, Pixz, Piyy, Piyz, Phi), 9 y-flux, 3 x 10 ring (n, w3, E6), 2 smoothing = 51 planes = 204 KB.
+// Collisionless component: fields n, nu (3), nE_ij (6: xx xy xz yy yz zz).
+// Shared planes (of PL doubles): primitives (n,ux) (uy,uz) (Pxx,Pxz) (Pyy,Pyz) pairs 8 + Pxy 1 +
+// Phi 1, y-flux (Ps0,Ps1) (Ps2,EF0) (EF1,EF2) (EF3,EF4) pairs 8 + EF5 1, ring 3 x 5 pair planes = 30,
+// z-averaged (w*_x,w*_y) pair 2  ->  51 planes = 204 KB.
 // =================================================================================================
-constexpr int BME_NR = 10;
-constexpr int BME_PLANES = 10 + 9 + 3 * BME_NR + 2;
+constexpr int BME_SLOT = 5 * PP;
+constexpr int BME_PLANES = 10 + 9 + 3 * 10 + 2;
+
+struct BmeCarry {
+    double n, in, u[3], Pi[6];            // primitives of the current plane j (own cell)
+    double acc[9];                        // U*(j) under construction: nu (3), nE (6)
+    double phi0, phim, phin;              // Phi(j), Phi(j-1), Phi(j+1) of the own column
+    double Sz_prev, wzp_prev, smax;
+    int bad;
+};
+
+struct BmeShared {
+    double *nu, *uu, *px, *py, *pxy, *phi, *fy, *ring, *tz;
+};
+
+template <bool ST>
+__device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f, const PhiCol& pc, const BmeShared& S,
+                                         BmeCarry& c, int j, double tau, double th, double inv2h) {
+    const Geo& g = a.g;
+    const int t = f.t;
+    const bool zout = g.bcz == GP_BC_OUTFLOW;
+    const bool top_copy = !ST && zout && j == g.nz;
+    const bool bot_dup = !ST && zout && j == 0;
+    const bool do_out = ST || j - 1 >= f.z0;
+    const bool do_wzp = ST || j >= f.z0;
+    const bool stage_next = ST || j + 1 <= f.z1;
+
+    // B: x and y faces of plane j (hi face per thread)
+    double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double gx = 0.0, gy = 0.0;
+    if (f.ty <= FY - 2) {
+        const int tr = t + FX;
+        const double2 r0 = lds2(S.nu + 2 * tr), r1 = lds2(S.uu + 2 * tr), r2 = lds2(S.py + 2 * tr);
+        const double ur[3] = {r0.y, r1.x, r1.y};
+        const double Pl[3] = {c.Pi[1], c.Pi[3], c.Pi[4]};
+        const double Pr[3] = {S.pxy[tr], r2.x, r2.y};
+        bme_face<1>(c.n, c.u, Pl, r0.x, ur, Pr, Py, EFy);
+        double* fy = S.fy;
+        sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
+        sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
+        fy[4 * PP + t] = EFy[5];
+    }
+    if (f.star_row) {
+        const int tr = f.tx < FX - 1 ? t + 1 : t;
+        const double2 r0 = lds2(S.nu + 2 * tr), r1 = lds2(S.uu + 2 * tr), r2 = lds2(S.px + 2 * tr);
+        const double ur[3] = {r0.y, r1.x, r1.y};
+        const double Pl[3] = {c.Pi[0], c.Pi[1], c.Pi[2]};
+        const double Pr[3] = {r2.x, S.pxy[tr], r2.y};
+        double Px[3], EFx[6];
+        bme_face<0>(c.n, c.u, Pl, r0.x, ur, Pr, Px, EFx);
+#pragma unroll
+        for (int q = 0; q < 3; ++q) c.acc[q] -= th * (Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1));
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th * (EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1));
+        gx = (S.phi[t + 1] - S.phi[t - 1]) * inv2h;
+        gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
+    }
+    __syncthreads();
+
+    // C: y-flux difference, then everything of U*(j) but the upper z face
+    if (f.star_row) {
+        const double* fy = S.fy + 2 * (t - FX);
+        const double2 l0 = lds2(fy), l1 = lds2(fy + PP), l2 = lds2(fy + 2 * PP), l3 = lds2(fy + 3 * PP);
+        const double l4 = S.fy[4 * PP + t - FX];
+        c.acc[0] -= th * (Py[0] - l0.x); c.acc[1] -= th * (Py[1] - l0.y); c.acc[2] -= th * (Py[2] - l1.x);
+        c.acc[3] -= th * (EFy[0] - l1.y); c.acc[4] -= th * (EFy[1] - l2.x); c.acc[5] -= th * (EFy[2] - l2.y);
+        c.acc[6] -= th * (EFy[3] - l3.x); c.acc[7] -= th * (EFy[4] - l3.y); c.acc[8] -= th * (EFy[5] - l4);
+        // gravity (reading G5): -tau n g_i and -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
+        const double gr[3] = {gx, gy, (c.phin - c.phim) * inv2h};
+        double uc[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], c.u[d]);
+        const double tn = tau * c.n;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c.acc[d] = fma(-tn, gr[d], c.acc[d]);
+        c.acc[3] = fma(-tn, 2.0 * uc[0] * gr[0], c.acc[3]);
+        c.acc[4] = fma(-tn, fma(uc[0], gr[1], uc[1] * gr[0]), c.acc[4]);
+        c.acc[5] = fma(-tn, fma(uc[0], gr[2], uc[2] * gr[0]), c.acc[5]);
+        c.acc[6] = fma(-tn, 2.0 * uc[1] * gr[1], c.acc[6]);
+        c.acc[7] = fma(-tn, fma(uc[1], gr[2], uc[2] * gr[1]), c.acc[7]);
+        c.acc[8] = fma(-tn, 2.0 * uc[2] * gr[2], c.acc[8]);
+    }
+
+    // E: plane j+1 arrives; z face (j, j+1); U*(j) complete -> ring slot j; publish primitives(j+1)
+    double* rs = S.ring + ring_slot(j) * BME_SLOT;
+    cp_async_wait_all();
+    double Un[NBME];
+    {
+        const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t), s2 = lds2(rs + 2 * PP + 2 * t),
+                      s3 = lds2(rs + 3 * PP + 2 * t), s4 = lds2(rs + 4 * PP + 2 * t);
+        Un[0] = s0.x; Un[1] = s0.y; Un[2] = s1.x; Un[3] = s1.y; Un[4] = s2.x; Un[5] = s2.y;
+        Un[6] = s3.x; Un[7] = s3.y; Un[8] = s4.x; Un[9] = s4.y;
+    }
+    const double n_n = Un[0];
+    const double in_n = frcp(n_n);
+    const double u_n[3] = {Un[1] * in_n, Un[2] * in_n, Un[3] * in_n};
+    double Pi_n[6];
+    Pi_n[0] = fma(-Un[1], u_n[0], Un[4]); Pi_n[1] = fma(-Un[1], u_n[1], Un[5]); Pi_n[2] = fma(-Un[1], u_n[2], Un[6]);
+    Pi_n[3] = fma(-Un[2], u_n[1], Un[7]); Pi_n[4] = fma(-Un[2], u_n[2], Un[8]); Pi_n[5] = fma(-Un[3], u_n[2], Un[9]);
+    double Pz[3] = {0.0, 0.0, 0.0}, EFz[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (f.star_row) {
+        const double Pl[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
+        const double Pr[3] = {Pi_n[2], Pi_n[4], Pi_n[5]};
+        bme_face<2>(c.n, c.u, Pl, n_n, u_n, Pr, Pz, EFz);
+        double o[NBME];      // n, w (3), nE (6)
+        if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
+            const double* rq = S.ring + ring_slot(j - 1) * BME_SLOT;
+            const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t), q2 = lds2(rq + 2 * PP + 2 * t),
+                          q3 = lds2(rq + 3 * PP + 2 * t), q4 = lds2(rq + 4 * PP + 2 * t);
+            o[0] = q0.x; o[3] = q0.y; o[1] = q1.x; o[2] = q1.y; o[4] = q2.x; o[5] = q2.y; o[6] = q3.x; o[7] = q3.y;
+            o[8] = q4.x; o[9] = q4.y;
+        } else {
+            o[0] = c.n;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) o[1 + d] = fma(-th, Pz[d], c.acc[d]) * c.in;
+#pragma unroll
+            for (int q = 0; q < 6; ++q) o[4 + q] = fma(-th, EFz[q], c.acc[3 + q]);
+        }
+        sts2(rs + 2 * t, o[0], o[3]); sts2(rs + PP + 2 * t, o[1], o[2]); sts2(rs + 2 * PP + 2 * t, o[4], o[5]);
+        sts2(rs + 3 * PP + 2 * t, o[6], o[7]); sts2(rs + 4 * PP + 2 * t, o[8], o[9]);
+        if (bot_dup) {                        // outflow: U*(-1) := U*(0)
+            double* rg = S.ring + ring_slot(-1) * BME_SLOT;
+            sts2(rg + 2 * t, o[0], o[3]); sts2(rg + PP + 2 * t, o[1], o[2]); sts2(rg + 2 * PP + 2 * t, o[4], o[5]);
+            sts2(rg + 3 * PP + 2 * t, o[6], o[7]); sts2(rg + 4 * PP + 2 * t, o[8], o[9]);
+        }
+        if (do_out) {                         // z-average of w*_x, w*_y for plane j-1
+            const double2 wm = lds2(S.ring + ring_slot(j - 2) * BME_SLOT + PP + 2 * t);
+            const double2 w0 = lds2(S.ring + ring_slot(j - 1) * BME_SLOT + PP + 2 * t);
+            sts2(S.tz + 2 * t, avg3(wm.x, w0.x, o[1]), avg3(wm.y, w0.y, o[2]));
+        }
+    }
+    sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
+    sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1]; S.phi[t] = c.phin;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) c.acc[d] = fma(th, Pz[d], Un[1 + d]);
+#pragma unroll
+    for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(th, EFz[q], Un[4 + q]);
+    c.n = n_n; c.in = in_n;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) c.u[d] = u_n[d];
+#pragma unroll
+    for (int q = 0; q < 6; ++q) c.Pi[q] = Pi_n[q];
+    c.phim = c.phi0; c.phi0 = c.phin;
+    __syncthreads();
+
+    if (f.block_fix) {
+        if (f.fix) {
+#pragma unroll
+            for (int P = 0; P < 5; ++P) {
+                const double2 v = lds2(rs + P * PP + 2 * f.fix_src);
+                sts2(rs + P * PP + 2 * t, v.x, v.y);
+                if (bot_dup) sts2(S.ring + ring_slot(-1) * BME_SLOT + P * PP + 2 * t, v.x, v.y);
+            }
+            const double2 v = lds2(S.tz + 2 * f.fix_src);
+            sts2(S.tz + 2 * t, v.x, v.y);
+        }
+        __syncthreads();
+    }
+
+    // D: Lagrangian stage of plane j-1 (ring planes j-2, j-1, j)
+    if (f.out_row) {
+        const double* rp = rs;
+        const double Sz_new = avg9_wz(rp, t);
+        if (bot_dup) c.Sz_prev = Sz_new;
+        if (do_wzp) {
+            const double wzp = 0.5 * (c.Sz_prev + Sz_new);
+            if (do_out) {
+                const double* r0 = S.ring + ring_slot(j - 1) * BME_SLOT;
+                const double* rm = S.ring + ring_slot(j - 2) * BME_SLOT;
+                double wxm, wxp, wym, wyp;
+                face_vel_xy(S.tz, t, wxm, wxp, wym, wyp);
+                const LagCoef lc = lag_coef(th, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
+                double out[NBME];
+                lagrange_cell<6>(rm, r0, rp, t, lc, out);
+                if (f.is_out) {
+                    const size_t off = f.base + (size_t)(j - 1) * f.nxny;
+#pragma unroll
+                    for (int q = 0; q < NBME; ++q) a.Un[q][off] = out[q];
+                    // CFL of the new state (reading G4): |u_d| + sqrt(3 Pi_dd / n)
+                    const double inn = frcp(out[0]);
+                    const int dd[3] = {4, 7, 9};
+                    if (!(out[0] > 0.0)) c.bad = 1;
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) {
+                        const double ud = out[1 + d] * inn;
+                        const double Pdd = fma(-out[1 + d], ud, out[dd[d]]);
+                        const double c2 = 3.0 * Pdd * inn;
+                        const double s = fabs(ud) + c2 * frsqrt(c2);
+                        if (!(Pdd > 0.0) || !(s <= 1.7976931348623157e308)) c.bad = 1;
+                        c.smax = fmax(c.smax, s);
+                    }
+                }
+            }
+            c.wzp_prev = wzp;
+        }
+        c.Sz_prev = Sz_new;
+    }
+    // stage plane j+2 into the slot D just finished with (own column only); Phi(j+2) to a register
+    if (stage_next) {
+        const int zm = map_safe(j + 2, g.nz, g.bcz);
+        const size_t off = f.base + (size_t)zm * f.nxny;
+        double* st = S.ring + ring_slot(j + 1) * BME_SLOT + 2 * t;
+#pragma unroll
+        for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
+        c.phin = phi_load(pc, j + 2, zm, g.nz);
+    }
+    cp_async_commit();
+}
 
 __global__ void __launch_bounds__(PL, 1)
 k_fused_bme(FusedArgs<NBME> a) {
-    extern __shared__ double sm[];
-    double* s_n = sm;                 // prims: n, ux, uy, uz, Pxx, Pxy, Pxz, Pyy, Pyz, Phi
-    double* s_phi = sm + 9 * PL;
-    double* s_fl = sm + 10 * PL;      // y-flux: Ps[3], EF[6]
-    double* ring = sm + 19 * PL;
-    double* s_tx = ring + 3 * BME_NR * PL; double* s_ty = s_tx + PL;
+    extern __shared__ double2 sm2[];
+    double* sm = reinterpret_cast<double*>(sm2);
+    BmeShared S;
+    S.nu = sm; S.uu = sm + 2 * PL; S.px = sm + 4 * PL; S.py = sm + 6 * PL; S.pxy = sm + 8 * PL; S.phi = sm + 9 * PL;
+    S.fy = sm + 10 * PL; S.ring = sm + 19 * PL; S.tz = S.ring + 3 * BME_SLOT;
 
-    const Geo g = a.g;
+    const Geo& g = a.g;
     const Foot f = make_foot(g, a.zchunk);
     const int t = f.t;
     const double tau = a.dt_ptr ? *a.dt_ptr : a.dt_val;
     const double th = tau / a.h, inv2h = 0.5 / a.h;
     const PhiCol pc = phi_col(g, a.phi, f.xv, f.yv, f.xm, f.ym);
-    const bool zout = g.bcz == GP_BC_OUTFLOW;
 
-    double nx_[NBME], nphi;
-    {
-        const int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
-        const size_t off = f.base + (size_t)zm * f.nxny;
+    BmeCarry c;
+    c.Sz_prev = c.wzp_prev = c.smax = 0.0; c.bad = 0;
+    {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
+        int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
+        size_t off = f.base + (size_t)zm * f.nxny;
+        double U0[NBME];
 #pragma unroll
-        for (int q = 0; q < NBME; ++q) nx_[q] = a.U[q][off];
-        nphi = phi_load(pc, f.z0 - 2, zm, g.nz);
+        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
+        c.phim = phi_load(pc, f.z0 - 2, zm, g.nz);
+        const double n_a = U0[0];
+        double in = frcp(n_a);
+        const double u_a[3] = {U0[1] * in, U0[2] * in, U0[3] * in};
+        const double Pz_a[3] = {fma(-U0[1], u_a[2], U0[6]), fma(-U0[2], u_a[2], U0[8]), fma(-U0[3], u_a[2], U0[9])};
+        zm = map_safe(f.z0 - 1, g.nz, g.bcz);
+        off = f.base + (size_t)zm * f.nxny;
+#pragma unroll
+        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
+        c.phi0 = phi_load(pc, f.z0 - 1, zm, g.nz);
+        c.n = U0[0]; c.in = frcp(c.n);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c.u[d] = U0[1 + d] * c.in;
+        c.Pi[0] = fma(-U0[1], c.u[0], U0[4]); c.Pi[1] = fma(-U0[1], c.u[1], U0[5]); c.Pi[2] = fma(-U0[1], c.u[2], U0[6]);
+        c.Pi[3] = fma(-U0[2], c.u[1], U0[7]); c.Pi[4] = fma(-U0[2], c.u[2], U0[8]); c.Pi[5] = fma(-U0[3], c.u[2], U0[9]);
+        const double Pr[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
+        double Pz[3], EFz[6];
+        bme_face<2>(n_a, u_a, Pz_a, c.n, c.u, Pr, Pz, EFz);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c.acc[d] = fma(th, Pz[d], U0[1 + d]);
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(th, EFz[q], U0[4 + q]);
+        sts2(S.nu + 2 * t, c.n, c.u[0]); sts2(S.uu + 2 * t, c.u[1], c.u[2]); sts2(S.px + 2 * t, c.Pi[0], c.Pi[2]);
+        sts2(S.py + 2 * t, c.Pi[3], c.Pi[4]); S.pxy[t] = c.Pi[1]; S.phi[t] = c.phi0;
+        // stage plane z0 where U*(z0-1) will be written
+        zm = map_safe(f.z0, g.nz, g.bcz);
+        off = f.base + (size_t)zm * f.nxny;
+        double* st = S.ring + ring_slot(f.z0 - 1) * BME_SLOT + 2 * t;
+#pragma unroll
+        for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
+        c.phin = phi_load(pc, f.z0, zm, g.nz);
+        cp_async_commit();
     }
-    // previous plane (for the z-face and for finishing U*(kv-1))
-    double pr_n = 1.0, pr_in = 1.0, pr_u[3] = {0.0, 0.0, 0.0}, pr_Pz[3] = {0.0, 0.0, 1.0};
-    double pr_gx = 0.0, pr_gy = 0.0;
-    double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};     // nu (3), nE (6) of U*(kv-1) so far
-    double phi_m1 = 0.0, phi_m2 = 0.0;
-    double Sz_prev = 0.0, wzp_prev = 0.0, smax = 0.0;
-    int bad = 0;
+    __syncthreads();
 
-    for (int kv = f.z0 - 2; kv <= f.z1 + 1; ++kv) {
-        double Uc[NBME];
-#pragma unroll
-        for (int q = 0; q < NBME; ++q) Uc[q] = nx_[q];
-        const double phi = nphi;
-        if (kv <= f.z1) {
-            const int zm = map_safe(kv + 1, g.nz, g.bcz);
-            const size_t off = f.base + (size_t)zm * f.nxny;
-#pragma unroll
-            for (int q = 0; q < NBME; ++q) nx_[q] = a.U[q][off];
-            nphi = phi_load(pc, kv + 1, zm, g.nz);
-        }
-        // A: primitives (S0): u = nu/n, Pi_ij = nE_ij - n u_i u_j
-        const double n = Uc[0];
-        const double in = frcp(n);
-        double u[3] = {Uc[1] * in, Uc[2] * in, Uc[3] * in};
-        double Pi[6];
-        Pi[0] = fma(-Uc[1], u[0], Uc[4]); Pi[1] = fma(-Uc[1], u[1], Uc[5]); Pi[2] = fma(-Uc[1], u[2], Uc[6]);
-        Pi[3] = fma(-Uc[2], u[1], Uc[7]); Pi[4] = fma(-Uc[2], u[2], Uc[8]); Pi[5] = fma(-Uc[3], u[2], Uc[9]);
-        s_n[t] = n; s_n[PL + t] = u[0]; s_n[2 * PL + t] = u[1]; s_n[3 * PL + t] = u[2];
-        s_n[4 * PL + t] = Pi[0]; s_n[5 * PL + t] = Pi[1]; s_n[6 * PL + t] = Pi[2];
-        s_n[7 * PL + t] = Pi[3]; s_n[8 * PL + t] = Pi[4]; s_phi[t] = phi;
-        __syncthreads();
-
-        // B: faces
-        const bool xy_stage = kv >= f.z0 - 1 && kv <= f.z1;
-        const bool z_stage = kv >= f.z0 - 1;
-        double Py[3], EFy[6], Px[3], EFx[6], Pxl[3], EFxl[6], Pz[3], EFz[6];
-#pragma unroll
-        for (int q = 0; q < 3; ++q) { Py[q] = Px[q] = Pxl[q] = Pz[q] = 0.0; }
-#pragma unroll
-        for (int q = 0; q < 6; ++q) { EFy[q] = EFx[q] = EFxl[q] = EFz[q] = 0.0; }
-        if (xy_stage && f.ty <= FY - 2) {
-            const int tr = t + FX;
-            const double ur[3] = {s_n[PL + tr], s_n[2 * PL + tr], s_n[3 * PL + tr]};
-            const double Pl[3] = {Pi[1], Pi[3], Pi[4]};
-            const double Pr[3] = {s_n[5 * PL + tr], s_n[7 * PL + tr], s_n[8 * PL + tr]};
-            bme_face<1>(n, u, Pl, s_n[tr], ur, Pr, Py, EFy);
-#pragma unroll
-            for (int q = 0; q < 3; ++q) s_fl[q * PL + t] = Py[q];
-#pragma unroll
-            for (int q = 0; q < 6; ++q) s_fl[(3 + q) * PL + t] = EFy[q];
-        }
-        if (f.star_row) {
-            if (xy_stage) {
-                const int tr = f.tx < FX - 1 ? t + 1 : t;
-                const double ur[3] = {s_n[PL + tr], s_n[2 * PL + tr], s_n[3 * PL + tr]};
-                const double Pl[3] = {Pi[0], Pi[1], Pi[2]};
-                const double Pr[3] = {s_n[4 * PL + tr], s_n[5 * PL + tr], s_n[6 * PL + tr]};
-                bme_face<0>(n, u, Pl, s_n[tr], ur, Pr, Px, EFx);
-#pragma unroll
-                for (int q = 0; q < 3; ++q) Pxl[q] = __shfl_up_sync(0xffffffffu, Px[q], 1);
-#pragma unroll
-                for (int q = 0; q < 6; ++q) EFxl[q] = __shfl_up_sync(0xffffffffu, EFx[q], 1);
-            }
-            if (z_stage) {
-                const double Pr[3] = {Pi[2], Pi[4], Pi[5]};
-                bme_face<2>(pr_n, pr_u, pr_Pz, n, u, Pr, Pz, EFz);
-            }
-        }
-        __syncthreads();
-
-        // C: finish U*(kv-1), start U*(kv)
-        if (f.star_row) {
-            if (kv >= f.z0) {
-                double* rs = ring + ring_slot(kv - 1) * BME_NR * PL;
-                if (zout && kv - 1 == g.nz) {
-                    const double* rq = ring + ring_slot(kv - 2) * BME_NR * PL;
-#pragma unroll
-                    for (int q = 0; q < BME_NR; ++q) rs[q * PL + t] = rq[q * PL + t];
-                } else {
-                    const double gr[3] = {pr_gx, pr_gy, (phi - phi_m2) * inv2h};
-                    double uc[3];       // time-centred velocity u - tau g / 2 (reading G5)
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], pr_u[d]);
-                    const double tn = tau * pr_n;
-                    double o[BME_NR];
-                    o[0] = pr_n;
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) o[1 + d] = (acc[d] - th * Pz[d] - tn * gr[d]) * pr_in;
-                    o[4] = acc[3] - th * EFz[0] - tn * (2.0 * uc[0] * gr[0]);
-                    o[5] = acc[4] - th * EFz[1] - tn * fma(uc[0], gr[1], uc[1] * gr[0]);
-                    o[6] = acc[5] - th * EFz[2] - tn * fma(uc[0], gr[2], uc[2] * gr[0]);
-                    o[7] = acc[6] - th * EFz[3] - tn * (2.0 * uc[1] * gr[1]);
-                    o[8] = acc[7] - th * EFz[4] - tn * fma(uc[1], gr[2], uc[2] * gr[1]);
-                    o[9] = acc[8] - th * EFz[5] - tn * (2.0 * uc[2] * gr[2]);
-#pragma unroll
-                    for (int q = 0; q < BME_NR; ++q) rs[q * PL + t] = o[q];
-                    if (zout && kv - 1 == 0) {
-                        double* rg = ring + ring_slot(-1) * BME_NR * PL;
-#pragma unroll
-                        for (int q = 0; q < BME_NR; ++q) rg[q * PL + t] = o[q];
-                    }
-                }
-            }
-            if (xy_stage) {
-                acc[0] = Uc[1] - th * ((Px[0] - Pxl[0]) + (Py[0] - s_fl[0 * PL + t - FX])) + th * Pz[0];
-                acc[1] = Uc[2] - th * ((Px[1] - Pxl[1]) + (Py[1] - s_fl[1 * PL + t - FX])) + th * Pz[1];
-                acc[2] = Uc[3] - th * ((Px[2] - Pxl[2]) + (Py[2] - s_fl[2 * PL + t - FX])) + th * Pz[2];
-#pragma unroll
-                for (int q = 0; q < 6; ++q)
-                    acc[3 + q] = Uc[4 + q] - th * ((EFx[q] - EFxl[q]) + (EFy[q] - s_fl[(3 + q) * PL + t - FX])) + th * EFz[q];
-                pr_gx = (s_phi[t + 1] - s_phi[t - 1]) * inv2h;
-                pr_gy = (s_phi[t + FX] - s_phi[t - FX]) * inv2h;
-            }
-        }
-        pr_n = n; pr_in = in;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) pr_u[d] = u[d];
-        pr_Pz[0] = Pi[2]; pr_Pz[1] = Pi[4]; pr_Pz[2] = Pi[5];
-        phi_m2 = phi_m1; phi_m1 = phi;
-        __syncthreads();
-
-        if (kv < f.z0) continue;
-        if (f.block_fix) {
-            if (f.fix) {
-                double* rs = ring + ring_slot(kv - 1) * BME_NR * PL;
-#pragma unroll
-                for (int q = 0; q < BME_NR; ++q) rs[q * PL + t] = rs[q * PL + f.fix_src];
-                if (zout && kv - 1 == 0) {
-                    double* rg = ring + ring_slot(-1) * BME_NR * PL;
-#pragma unroll
-                    for (int q = 0; q < BME_NR; ++q) rg[q * PL + t] = rg[q * PL + f.fix_src];
-                }
-            }
-            __syncthreads();
-        }
-
-        // D: Lagrangian stage of plane k = kv-2
-        const double* rp = ring + ring_slot(kv - 1) * BME_NR * PL;
-        const double* r0 = ring + ring_slot(kv - 2) * BME_NR * PL;
-        const double* rm = ring + ring_slot(kv - 3) * BME_NR * PL;
-        const bool do_out = kv >= f.z0 + 2;
-        if (do_out && f.star_row) {
-            s_tx[t] = avg3(rm[PL + t], r0[PL + t], rp[PL + t]);
-            s_ty[t] = avg3(rm[2 * PL + t], r0[2 * PL + t], rp[2 * PL + t]);
-        }
-        if (do_out) __syncthreads();
-        if (f.out_row) {
-            const double Sz_new = avg9(rp + 3 * PL, t);
-            if (zout && kv - 1 == 0) Sz_prev = Sz_new;
-            if (kv >= f.z0 + 1) {
-                const double wzp = 0.5 * (Sz_prev + Sz_new);
-                if (do_out) {
-                    const double a_m = avg3(s_tx[t - FX - 1], s_tx[t - 1], s_tx[t + FX - 1]);
-                    const double a_0 = avg3(s_tx[t - FX], s_tx[t], s_tx[t + FX]);
-                    const double a_p = avg3(s_tx[t - FX + 1], s_tx[t + 1], s_tx[t + FX + 1]);
-                    const double b_m = avg3(s_ty[t - FX - 1], s_ty[t - FX], s_ty[t - FX + 1]);
-                    const double b_0 = avg3(s_ty[t - 1], s_ty[t], s_ty[t + 1]);
-                    const double b_p = avg3(s_ty[t + FX - 1], s_ty[t + FX], s_ty[t + FX + 1]);
-                    double out[NBME];
-                    lagrange_cell<6>(rm, r0, rp, t, th, 0.5 * (a_m + a_0), 0.5 * (a_0 + a_p), 0.5 * (b_m + b_0),
-                                     0.5 * (b_0 + b_p), wzp_prev, wzp, out);
-                    if (f.is_out) {
-                        const size_t off = f.base + (size_t)(kv - 2) * f.nxny;
-#pragma unroll
-                        for (int q = 0; q < NBME; ++q) a.Un[q][off] = out[q];
-                        // CFL of the new state (reading G4): |u_d| + sqrt(3 Pi_dd / n)
-                        const double inn = frcp(out[0]);
-                        const int dd[3] = {4, 7, 9};
-                        if (!(out[0] > 0.0)) bad = 1;
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) {
-                            const double ud = out[1 + d] * inn;
-                            const double Pdd = fma(-out[1 + d], ud, out[dd[d]]);
-                            const double c2 = 3.0 * Pdd * inn;
-                            const double s = fabs(ud) + c2 * frsqrt(c2);
-                            if (!(Pdd > 0.0) || !(s <= 1.7976931348623157e308)) bad = 1;
-                            smax = fmax(smax, s);
-                        }
-                    }
-                }
-                wzp_prev = wzp;
-            }
-            Sz_prev = Sz_new;
-        }
-    }
-    block_max_commit(smax, bad, a.smax_bits, a.flag, s_n);
+    int j = f.z0 - 1;
+    for (; j <= f.z0 && j <= f.z1; ++j) bme_iter<false>(a, f, pc, S, c, j, tau, th, inv2h);
+    for (; j <= f.z1 - 1; ++j) bme_iter<true>(a, f, pc, S, c, j, tau, th, inv2h);
+    for (; j <= f.z1; ++j) bme_iter<false>(a, f, pc, S, c, j, tau, th, inv2h);
+    cp_async_wait_all();
+    block_max_commit(c.smax, c.bad, a.smax_bits, a.flag, S.nu);
 }
 
 // -------------------------------------------------------------------------------------------------
