@@ -87,56 +87,60 @@ __device__ __forceinline__ const double* phi_ptr(const PhiCol& c, int kv, int zm
 __device__ __forceinline__ double phi_load(const PhiCol& c, int kv, int zm, int nz) { return *phi_ptr(c, kv, zm, nz); }
 
 // ---- face solvers ------------------------------------------------------------------------------
+// The solvers return DOUBLED face values (2P, 4PV ...) so that the factors 1/2 of the paper's
+// formulas fold into the flux coefficients tau/(2h), tau/(4h) (exact power-of-two scalings).
+//
 // PAPER.md:112, 114 with Z = sqrt(rl rr gamma (pl+pr)/(rl+rr)) = num*r, 1/Z = den*r, r = rsqrt(num*den).
+// Out: P2 = 2P, PV4 = 4 P V.
 __device__ __forceinline__ void gas_face(double gamma, double rl, double vl, double pl, double rr, double vr, double pr,
-                                         double& P, double& PV) {
+                                         double& P2, double& PV4) {
     const double ps = pl + pr;
     const double num = rl * rr * (gamma * ps), den = rl + rr;
     const double r = frsqrt(num * den);
     const double Z = num * r, iZ = den * r;
-    const double V = fma(0.5 * (pl - pr), iZ, 0.5 * (vl + vr));
-    P = fma(0.5 * (vl - vr), Z, 0.5 * ps);
-    PV = P * V;
+    const double V2 = fma(pl - pr, iZ, vl + vr);
+    P2 = fma(vl - vr, Z, ps);
+    PV4 = P2 * V2;
 }
 
 // PAPER.md:170-178 for a face normal to axis D, bracketed parameters averaged (PAPER.md:180,
 // reading G7).  In: n, u[3], Pd[3] = Pi_{xD}, Pi_{yD}, Pi_{zD} of both sides.
-// Out: Ps[3] = Pi*_{.D} (momentum flux) and EF[6] = Pi*_{jD} u*_i + Pi*_{iD} u*_j for
+// Out: Ps2[3] = 2 Pi*_{.D} (momentum flux) and EF4[6] = 4 (Pi*_{jD} u*_i + Pi*_{iD} u*_j) for
 // (i,j) = xx xy xz yy yz zz (flux of nE_ij).
-// With q = 2 nl nr, s = nl+nr, a = (Pl+Pr)/2:  [rho] = q/s, Z1 = sqrt([rho] a) = q a r,
-// 1/Z1 = s r, 1/a = q s r^2, where r = rsqrt(q a s).
+// With q = nl nr, s = nl+nr, A = Pl+Pr (= 2a):  [rho] a = q A / s,  Z1 = sqrt([rho] a) = q A r,
+// 1/Z1 = s r, 1/a = 2 q s r^2, where r = rsqrt(q A s).
 template <int D>
 __device__ __forceinline__ void bme_face(double nl, const double ul[3], const double Pl[3],
                                          double nr, const double ur[3], const double Pr[3],
-                                         double Ps[3], double EF[6]) {
+                                         double Ps2[3], double EF4[6]) {
     const double s3 = 1.7320508075688772935, is3 = 0.57735026918962576451;
-    const double q = (nl + nl) * nr, s = nl + nr;
-    const double a = 0.5 * (Pl[D] + Pr[D]);
-    const double qa = q * a;
-    const double r = frsqrt(qa * s);
-    const double Z1 = qa * r, iZ1 = s * r;
-    const double ia = (q * s) * (r * r);
+    const double q = nl * nr, s = nl + nr;
+    const double A = Pl[D] + Pr[D];
+    const double qA = q * A;
+    const double r = frsqrt(qA * s);
+    const double Z1 = qA * r, iZ1 = s * r;
+    const double ia = (q * s) * (2.0 * r * r);
     const double Z3 = s3 * Z1, iZ3 = is3 * iZ1;
-    const double dPdd = 0.5 * (Pl[D] - Pr[D]);
-    const double dud = 0.5 * (ul[D] - ur[D]);
-    double us[3];
-    us[D] = fma(dPdd, iZ3, 0.5 * (ul[D] + ur[D]));
-    Ps[D] = fma(dud, Z3, a);
-    const double ku = (1.0 - s3) * (ia * iZ3) * dPdd;      // dPdd (1-sqrt3) / (a Z3)
-    const double kp = (s3 - 1.0) * (Z1 * ia) * dud;        // dud [rho] (sqrt3-1) / Z1 = dud (sqrt3-1) Z1 / a
+    const double DP = Pl[D] - Pr[D], DU = ul[D] - ur[D];
+    double us2[3];
+    us2[D] = fma(DP, iZ3, ul[D] + ur[D]);
+    Ps2[D] = fma(DU, Z3, A);
+    // b ku = (B/2) (1-sqrt3) (DP/2) / (a Z3) and doubled: B * [(1-sqrt3)/2 * ia * iZ3 * DP]
+    const double ku = (0.5 * (1.0 - s3)) * (ia * iZ3) * DP;
+    const double kp = (0.5 * (s3 - 1.0)) * (Z1 * ia) * DU;
 #pragma unroll
     for (int w = 1; w <= 2; ++w) {
         const int t = (D + w) % 3;
-        const double b = 0.5 * (Pl[t] + Pr[t]);
-        us[t] = fma(b, ku, fma(0.5 * (Pl[t] - Pr[t]), iZ1, 0.5 * (ul[t] + ur[t])));
-        Ps[t] = fma(b, kp, fma(0.5 * (ul[t] - ur[t]), Z1, b));
+        const double B = Pl[t] + Pr[t];
+        us2[t] = fma(B, ku, fma(Pl[t] - Pr[t], iZ1, ul[t] + ur[t]));
+        Ps2[t] = fma(B, kp, fma(ul[t] - ur[t], Z1, B));
     }
-    EF[0] = 2.0 * Ps[0] * us[0];
-    EF[1] = fma(Ps[1], us[0], Ps[0] * us[1]);
-    EF[2] = fma(Ps[2], us[0], Ps[0] * us[2]);
-    EF[3] = 2.0 * Ps[1] * us[1];
-    EF[4] = fma(Ps[2], us[1], Ps[1] * us[2]);
-    EF[5] = 2.0 * Ps[2] * us[2];
+    EF4[0] = 2.0 * Ps2[0] * us2[0];
+    EF4[1] = fma(Ps2[1], us2[0], Ps2[0] * us2[1]);
+    EF4[2] = fma(Ps2[2], us2[0], Ps2[0] * us2[2]);
+    EF4[3] = 2.0 * Ps2[1] * us2[1];
+    EF4[4] = fma(Ps2[2], us2[1], Ps2[1] * us2[2]);
+    EF4[5] = 2.0 * Ps2[2] * us2[2];
 }
 
 // ---- shared-memory helpers ---------------------------------------------------------------------
@@ -149,61 +153,82 @@ __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const double* gmem) { asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem)); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// (1/4,1/2,1/4) average of three values
-__device__ __forceinline__ double avg3(double a, double b, double c) { return fma(0.25, a + c, 0.5 * b); }
+// 4 x the (1/4,1/2,1/4) average of three values; the power-of-two normalisations of the face
+// velocity (reading G2: 1/4 * 1/4 * 1/2 = 1/32) fold into the flux coefficient (lag_coef).
+__device__ __forceinline__ double sum3(double a, double b, double c) { return fma(2.0, b, a + c); }
 
 // Ring slot layout (doubles): pair plane P at offset P*2*PL, cell t at 2*t, two fields per cell:
 //   P0 = (density, w*_z)   P1 = (w*_x, w*_y)   P2.. = the remaining fields in pairs
 // so that every neighbour access is one 128-bit load.
 constexpr int PP = 2 * PL;   // doubles per pair plane
 
-// 3x3 (omega x omega) average of the second member of pair plane P0 (w*_z) around cell t
-__device__ __forceinline__ double avg9_wz(const double* __restrict__ r, int t) {
+// 16 x the 3x3 (omega x omega) average of the second member of pair plane P0 (w*_z) around cell t
+__device__ __forceinline__ double sum9_wz(const double* __restrict__ r, int t) {
     const double* s = r + 1;
-    const double lo = avg3(s[2 * (t - FX - 1)], s[2 * (t - FX)], s[2 * (t - FX + 1)]);
-    const double mi = avg3(s[2 * (t - 1)], s[2 * t], s[2 * (t + 1)]);
-    const double hi = avg3(s[2 * (t + FX - 1)], s[2 * (t + FX)], s[2 * (t + FX + 1)]);
-    return avg3(lo, mi, hi);
+    const double lo = sum3(s[2 * (t - FX - 1)], s[2 * (t - FX)], s[2 * (t - FX + 1)]);
+    const double mi = sum3(s[2 * (t - 1)], s[2 * t], s[2 * (t + 1)]);
+    const double hi = sum3(s[2 * (t + FX - 1)], s[2 * (t + FX)], s[2 * (t + FX + 1)]);
+    return sum3(lo, mi, hi);
 }
 
 // Upwind flux form of one cell in coefficient form:
 //   F+ = max(w+,0) f0 + min(w+,0) f+,  F- = max(w-,0) f- + min(w-,0) f0,
 //   f' = f0 - th (sum_d F+ - F-) = c0 f0 + sum_q c_q f_q,   max(w,0) = (w+|w|)/2, min(w,0) = (w-|w|)/2.
+// The face velocities come in as W = 32 w (unnormalised sums), so the coefficient is th/64.
 struct LagCoef { double c0, xm, xp, ym, yp, zm, zp; };
 
-__device__ __forceinline__ LagCoef lag_coef(double th, double wxm, double wxp, double wym, double wyp, double wzm, double wzp) {
-    const double hth = 0.5 * th;
+__device__ __forceinline__ LagCoef lag_coef(double th64, double wxm, double wxp, double wym, double wyp, double wzm, double wzp) {
     LagCoef c;
-    c.xm = hth * (wxm + fabs(wxm)); c.xp = hth * (fabs(wxp) - wxp);
-    c.ym = hth * (wym + fabs(wym)); c.yp = hth * (fabs(wyp) - wyp);
-    c.zm = hth * (wzm + fabs(wzm)); c.zp = hth * (fabs(wzp) - wzp);
+    c.xm = th64 * (wxm + fabs(wxm)); c.xp = th64 * (fabs(wxp) - wxp);
+    c.ym = th64 * (wym + fabs(wym)); c.yp = th64 * (fabs(wyp) - wyp);
+    c.zm = th64 * (wzm + fabs(wzm)); c.zp = th64 * (fabs(wzp) - wzp);
     const double sum = ((wxp + fabs(wxp)) + (fabs(wxm) - wxm)) + ((wyp + fabs(wyp)) + (fabs(wym) - wym)) +
                        ((wzp + fabs(wzp)) + (fabs(wzm) - wzm));
-    c.c0 = fma(-hth, sum, 1.0);
+    c.c0 = fma(-th64, sum, 1.0);
     return c;
 }
 
-// Lagrangian stage of one output cell from the U* ring.  Momentum = density * w*, so its update is
+// Lagrangian stage of one output cell from the U* ring, in two parts so that the ring slot of
+// plane j-2 (read only at the thread's own column) can be handed to the asynchronous staging of
+// the next plane as early as possible.  Momentum = density * w*, so its update is
 // sum_q (c_q dens_q) w*_q.  out = (density, momentum x y z, NO remaining fields).
 template <int NO>
-__device__ __forceinline__ void lagrange_cell(const double* __restrict__ rm, const double* __restrict__ r0,
-                                              const double* __restrict__ rp, int t, const LagCoef& c, double out[4 + NO]) {
+__device__ __forceinline__ void lagrange_lower(const double* __restrict__ rm, int t, const LagCoef& c, double out[4 + NO]) {
+    const double2 azm = lds2(rm + 2 * t), bzm = lds2(rm + PP + 2 * t);
+    const double dzm = c.zm * azm.x;
+    out[0] = dzm; out[3] = dzm * azm.y; out[1] = dzm * bzm.x; out[2] = dzm * bzm.y;
+#pragma unroll
+    for (int P = 0; P < (NO + 1) / 2; ++P) {
+        const int o = (2 + P) * PP;
+        if (2 * P + 1 < NO) {
+            const double2 ezm = lds2(rm + o + 2 * t);
+            out[4 + 2 * P] = c.zm * ezm.x; out[5 + 2 * P] = c.zm * ezm.y;
+        } else {
+            out[4 + 2 * P] = c.zm * rm[o + 2 * t];
+        }
+    }
+}
+
+template <int NO>
+__device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, const double* __restrict__ rp, int t,
+                                              const LagCoef& c, double out[4 + NO]) {
     const double2 a0 = lds2(r0 + 2 * t), axm = lds2(r0 + 2 * (t - 1)), axp = lds2(r0 + 2 * (t + 1));
     const double2 aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
-    const double2 azm = lds2(rm + 2 * t), azp = lds2(rp + 2 * t);
+    const double2 azp = lds2(rp + 2 * t);
     const double d0 = c.c0 * a0.x, dxm = c.xm * axm.x, dxp = c.xp * axp.x, dym = c.ym * aym.x, dyp = c.yp * ayp.x,
-                 dzm = c.zm * azm.x, dzp = c.zp * azp.x;
-    out[0] = ((d0 + dxm) + (dxp + dym)) + ((dyp + dzm) + dzp);
-    out[3] = fma(dzp, azp.y, fma(dzm, azm.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, d0 * a0.y))))));
+                 dzp = c.zp * azp.x;
+    out[0] = ((out[0] + d0) + (dxm + dxp)) + ((dym + dyp) + dzp);
+    out[3] = fma(dzp, azp.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, fma(d0, a0.y, out[3]))))));
     {
         const double2 b0 = lds2(r0 + PP + 2 * t), bxm = lds2(r0 + PP + 2 * (t - 1)), bxp = lds2(r0 + PP + 2 * (t + 1));
         const double2 bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
-        const double2 bzm = lds2(rm + PP + 2 * t), bzp = lds2(rp + PP + 2 * t);
-        out[1] = fma(dzp, bzp.x, fma(dzm, bzm.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, d0 * b0.x))))));
-        out[2] = fma(dzp, bzp.y, fma(dzm, bzm.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, d0 * b0.y))))));
+        const double2 bzp = lds2(rp + PP + 2 * t);
+        out[1] = fma(dzp, bzp.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, fma(d0, b0.x, out[1]))))));
+        out[2] = fma(dzp, bzp.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, fma(d0, b0.y, out[2]))))));
     }
 #pragma unroll
     for (int P = 0; P < (NO + 1) / 2; ++P) {
@@ -211,29 +236,29 @@ __device__ __forceinline__ void lagrange_cell(const double* __restrict__ rm, con
         if (2 * P + 1 < NO) {
             const double2 e0 = lds2(r0 + o + 2 * t), exm = lds2(r0 + o + 2 * (t - 1)), exp_ = lds2(r0 + o + 2 * (t + 1));
             const double2 eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
-            const double2 ezm = lds2(rm + o + 2 * t), ezp = lds2(rp + o + 2 * t);
-            out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.zm, ezm.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, c.c0 * e0.x))))));
-            out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.zm, ezm.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, c.c0 * e0.y))))));
+            const double2 ezp = lds2(rp + o + 2 * t);
+            out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, fma(c.c0, e0.x, out[4 + 2 * P]))))));
+            out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, fma(c.c0, e0.y, out[5 + 2 * P]))))));
         } else {
             const double e0 = r0[o + 2 * t], exm = r0[o + 2 * (t - 1)], exp_ = r0[o + 2 * (t + 1)];
             const double eym = r0[o + 2 * (t - FX)], eyp = r0[o + 2 * (t + FX)];
-            const double ezm = rm[o + 2 * t], ezp = rp[o + 2 * t];
-            out[4 + 2 * P] = fma(c.zp, ezp, fma(c.zm, ezm, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, c.c0 * e0))))));
+            const double ezp = rp[o + 2 * t];
+            out[4 + 2 * P] = fma(c.zp, ezp, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, fma(c.c0, e0, out[4 + 2 * P]))))));
         }
     }
 }
 
-// Face velocities of one output cell (reading G2) from the z-averaged w*_x, w*_y pair plane
-// (s_tz) : x faces = mean of the y-averaged columns tx-1|tx and tx|tx+1, y faces likewise.
+// 32 x the face velocities of one output cell (reading G2) from the z-summed (4 x averaged) w*_x,
+// w*_y pair plane (s_tz): x faces = sum of the y-summed columns tx-1|tx and tx|tx+1, y faces likewise.
 __device__ __forceinline__ void face_vel_xy(const double* __restrict__ s_tz, int t, double& wxm, double& wxp, double& wym,
                                             double& wyp) {
     const double2 mm = lds2(s_tz + 2 * (t - FX - 1)), m0 = lds2(s_tz + 2 * (t - FX)), mp = lds2(s_tz + 2 * (t - FX + 1));
     const double2 zm = lds2(s_tz + 2 * (t - 1)), z0 = lds2(s_tz + 2 * t), zp = lds2(s_tz + 2 * (t + 1));
     const double2 pm = lds2(s_tz + 2 * (t + FX - 1)), p0 = lds2(s_tz + 2 * (t + FX)), pp = lds2(s_tz + 2 * (t + FX + 1));
-    const double a_m = avg3(mm.x, zm.x, pm.x), a_0 = avg3(m0.x, z0.x, p0.x), a_p = avg3(mp.x, zp.x, pp.x);
-    const double b_m = avg3(mm.y, m0.y, mp.y), b_0 = avg3(zm.y, z0.y, zp.y), b_p = avg3(pm.y, p0.y, pp.y);
-    wxm = 0.5 * (a_m + a_0); wxp = 0.5 * (a_0 + a_p);
-    wym = 0.5 * (b_m + b_0); wyp = 0.5 * (b_0 + b_p);
+    const double a_m = sum3(mm.x, zm.x, pm.x), a_0 = sum3(m0.x, z0.x, p0.x), a_p = sum3(mp.x, zp.x, pp.x);
+    const double b_m = sum3(mm.y, m0.y, mp.y), b_0 = sum3(zm.y, z0.y, zp.y), b_p = sum3(pm.y, p0.y, pp.y);
+    wxm = a_m + a_0; wxp = a_0 + a_p;
+    wym = b_m + b_0; wyp = b_0 + b_p;
 }
 
 template <int NF>
@@ -341,6 +366,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
     const Geo& g = a.g;
     const int t = f.t;
     const double gamma = a.gamma, gm1 = a.gamma - 1.0;
+    const double th2 = 0.5 * th, th4 = 0.25 * th;
     const bool zout = g.bcz == GP_BC_OUTFLOW;
     const bool top_copy = !ST && zout && j == g.nz;
     const bool bot_dup = !ST && zout && j == 0;
@@ -348,26 +374,27 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
     const bool do_wzp = ST || j >= f.z0;
     const bool stage_next = ST || j + 1 <= f.z1;
 
-    // B: x and y faces of plane j (each computed once: hi face per thread)
+    // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
+    // that the two solvers interleave.  Row FY-1 has no row above it; its faces are never used.
     double Pyh = 0.0, PVyh = 0.0, gy = 0.0;
     if (f.ty <= FY - 2) {
-        const double2 r = lds2(S.rp + 2 * (t + FX));
-        gas_face(gamma, c.rho, c.vy, c.p, r.x, S.vy[t + FX], r.y, Pyh, PVyh);
-        sts2(S.fy + 2 * t, Pyh, PVyh);
-    }
-    if (f.star_row) {
         const int tr = f.tx < FX - 1 ? t + 1 : t;
-        const double2 r = lds2(S.rp + 2 * tr);
+        const double2 ry = lds2(S.rp + 2 * (t + FX)), rx = lds2(S.rp + 2 * tr);
+        const double vyr = S.vy[t + FX], vxr = S.vx[tr];
+        const double phe = S.phi[tr], phn = S.phi[t + FX];
+        const double phw = S.phi[f.tx > 0 ? t - 1 : t], phs = S.phi[f.ty > 0 ? t - FX : t];
         double Pxh, PVxh;
-        gas_face(gamma, c.rho, c.vx, c.p, r.x, S.vx[tr], r.y, Pxh, PVxh);
+        gas_face(gamma, c.rho, c.vy, c.p, ry.x, vyr, ry.y, Pyh, PVyh);
+        gas_face(gamma, c.rho, c.vx, c.p, rx.x, vxr, rx.y, Pxh, PVxh);
+        sts2(S.fy + 2 * t, Pyh, PVyh);
         const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1);
         const double PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
-        const double gx = (S.phi[t + 1] - S.phi[t - 1]) * inv2h;
-        gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
+        const double gx = (phe - phw) * inv2h;
+        gy = (phn - phs) * inv2h;
         const double trg = tau * c.rho * gx;
         const double mx = c.rho * c.vx;
-        c.amx = c.amx - th * (Pxh - Pxl) - trg;
-        c.aE = c.aE - th * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
+        c.amx = c.amx - th2 * (Pxh - Pxl) - trg;
+        c.aE = c.aE - th4 * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
     }
     __syncthreads();
 
@@ -376,8 +403,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
         const double2 lo = lds2(S.fy + 2 * (t - FX));
         const double trg = tau * c.rho * gy;
         const double my = c.rho * c.vy;
-        c.amy = c.amy - th * (Pyh - lo.x) - trg;
-        c.aE = c.aE - th * (PVyh - lo.y) - fma(-0.5 * tau, trg, tau * my) * gy;
+        c.amy = c.amy - th2 * (Pyh - lo.x) - trg;
+        c.aE = c.aE - th4 * (PVyh - lo.y) - fma(-0.5 * tau, trg, tau * my) * gy;
     }
 
     // E: plane j+1 arrives; z face (j, j+1); U*(j) complete -> ring slot j; publish primitives(j+1)
@@ -400,8 +427,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
             const double gz = (phi_n - c.phim) * inv2h;
             const double trg = tau * c.rho * gz;
             const double mz = c.rho * c.vz;
-            const double mzs = c.amz - th * Pz - trg;
-            Es = c.aE - th * PVz - fma(-0.5 * tau, trg, tau * mz) * gz;
+            const double mzs = c.amz - th2 * Pz - trg;
+            Es = c.aE - th4 * PVz - fma(-0.5 * tau, trg, tau * mz) * gz;
             dens = c.rho; wx = c.amx * c.ir; wy = c.amy * c.ir; wz = mzs * c.ir;
         }
         sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy); rs[2 * PP + 2 * t] = Es;
@@ -409,14 +436,14 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
             double* rg = S.ring + ring_slot(-1) * GAS_SLOT;
             sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy); rg[2 * PP + 2 * t] = Es;
         }
-        if (do_out) {                         // z-average of w*_x, w*_y for plane j-1
+        if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
             const double2 wm = lds2(S.ring + ring_slot(j - 2) * GAS_SLOT + PP + 2 * t);
             const double2 w0 = lds2(S.ring + ring_slot(j - 1) * GAS_SLOT + PP + 2 * t);
-            sts2(S.tz + 2 * t, avg3(wm.x, w0.x, wx), avg3(wm.y, w0.y, wy));
+            sts2(S.tz + 2 * t, sum3(wm.x, w0.x, wx), sum3(wm.y, w0.y, wy));
         }
     }
     sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n; S.phi[t] = phi_n;
-    c.amx = mx_n; c.amy = my_n; c.amz = fma(th, Pz, mz_n); c.aE = fma(th, PVz, E_n);
+    c.amx = mx_n; c.amy = my_n; c.amz = fma(th2, Pz, mz_n); c.aE = fma(th4, PVz, E_n);
     c.rho = rho_n; c.ir = ir_n; c.vx = vx_n; c.vy = vy_n; c.vz = vz_n; c.p = p_n;
     c.phim = c.phi0; c.phi0 = phi_n;
     __syncthreads();
@@ -435,40 +462,27 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
         __syncthreads();
     }
 
-    // D: Lagrangian stage of plane j-1 (ring planes j-2, j-1, j)
+    // D: Lagrangian stage of plane j-1 (ring planes j-2, j-1, j).  The slot of plane j-2 is read
+    // first (own column only) and then handed to the staging of plane j+2.
+    double out[NGAS];
+    LagCoef lc;
+    bool emit = false;
     if (f.out_row) {
-        const double* rp = rs;
-        const double Sz_new = avg9_wz(rp, t);
+        const double Sz_new = sum9_wz(rs, t);             // 16 x
         if (bot_dup) c.Sz_prev = Sz_new;
         if (do_wzp) {
-            const double wzp = 0.5 * (c.Sz_prev + Sz_new);
+            const double wzp = c.Sz_prev + Sz_new;        // 32 x face velocity between planes j-1 and j
             if (do_out) {
-                const double* r0 = S.ring + ring_slot(j - 1) * GAS_SLOT;
-                const double* rm = S.ring + ring_slot(j - 2) * GAS_SLOT;
                 double wxm, wxp, wym, wyp;
                 face_vel_xy(S.tz, t, wxm, wxp, wym, wyp);
-                const LagCoef lc = lag_coef(th, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
-                double out[NGAS];
-                lagrange_cell<1>(rm, r0, rp, t, lc, out);
-                if (f.is_out) {
-                    const size_t off = f.base + (size_t)(j - 1) * f.nxny;
-#pragma unroll
-                    for (int q = 0; q < NGAS; ++q) a.Un[q][off] = out[q];
-                    // CFL of the new state (reading G4)
-                    const double irn = frcp(out[0]);
-                    const double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
-                    const double pn = gm1 * (out[4] - 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz)));
-                    const double c2 = gamma * pn * irn;
-                    const double s = fmax(fmax(fabs(ux), fabs(uy)), fabs(uz)) + c2 * frsqrt(c2);
-                    if (!(out[0] > 0.0) || !(pn > 0.0) || !(s <= 1.7976931348623157e308)) c.bad = 1;
-                    c.smax = fmax(c.smax, s);
-                }
+                lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
+                lagrange_lower<1>(S.ring + ring_slot(j - 2) * GAS_SLOT, t, lc, out);
+                emit = true;
             }
             c.wzp_prev = wzp;
         }
         c.Sz_prev = Sz_new;
     }
-    // stage plane j+2 into the slot D just finished with (own column only)
     if (stage_next) {
         const int zm = map_safe(j + 2, g.nz, g.bcz);
         const size_t off = f.base + (size_t)zm * f.nxny;
@@ -479,6 +493,22 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
         cp_async8(st + 2 * PP + 2 * t + 1, phi_ptr(pc, j + 2, zm, g.nz));
     }
     cp_async_commit();
+    if (emit) {
+        lagrange_rest<1>(S.ring + ring_slot(j - 1) * GAS_SLOT, rs, t, lc, out);
+        if (f.is_out) {
+            const size_t off = f.base + (size_t)(j - 1) * f.nxny;
+#pragma unroll
+            for (int q = 0; q < NGAS; ++q) a.Un[q][off] = out[q];
+            // CFL of the new state (reading G4)
+            const double irn = frcp(out[0]);
+            const double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
+            const double pn = gm1 * (out[4] - 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz)));
+            const double c2 = gamma * pn * irn;
+            const double sp = fmax(fmax(fabs(ux), fabs(uy)), fabs(uz)) + c2 * frsqrt(c2);
+            if (!(out[0] > 0.0) || !(pn > 0.0) || !(sp <= 1.7976931348623157e308)) c.bad = 1;
+            c.smax = fmax(c.smax, sp);
+        }
+    }
 }
 
 __global__ void __launch_bounds__(PL, 1)
@@ -516,7 +546,7 @@ k_fused_gas(FusedArgs<NGAS> a) {
         c.p = gm1 * (E - 0.5 * fma(mx, c.vx, fma(my, c.vy, mz * c.vz)));
         double Pz, PVz;
         gas_face(a.gamma, rho_a, vz_a, p_a, c.rho, c.vz, c.p, Pz, PVz);
-        c.amx = mx; c.amy = my; c.amz = fma(th, Pz, mz); c.aE = fma(th, PVz, E);
+        c.amx = mx; c.amy = my; c.amz = fma(0.5 * th, Pz, mz); c.aE = fma(0.25 * th, PVz, E);
         c.phim = phi_a; c.phi0 = phi_b;
         sts2(S.rp + 2 * t, c.rho, c.p); S.vx[t] = c.vx; S.vy[t] = c.vy; S.phi[t] = phi_b;
         // stage plane z0 where U*(z0-1) will be written
@@ -565,6 +595,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
                                          BmeCarry& c, int j, double tau, double th, double inv2h) {
     const Geo& g = a.g;
     const int t = f.t;
+    const double th2 = 0.5 * th, th4 = 0.25 * th;
     const bool zout = g.bcz == GP_BC_OUTFLOW;
     const bool top_copy = !ST && zout && j == g.nz;
     const bool bot_dup = !ST && zout && j == 0;
@@ -576,29 +607,29 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
     double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     double gx = 0.0, gy = 0.0;
     if (f.ty <= FY - 2) {
-        const int tr = t + FX;
-        const double2 r0 = lds2(S.nu + 2 * tr), r1 = lds2(S.uu + 2 * tr), r2 = lds2(S.py + 2 * tr);
-        const double ur[3] = {r0.y, r1.x, r1.y};
+        const int tn = t + FX;
+        const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
+        const double ur[3] = {y0.y, y1.x, y1.y};
         const double Pl[3] = {c.Pi[1], c.Pi[3], c.Pi[4]};
-        const double Pr[3] = {S.pxy[tr], r2.x, r2.y};
-        bme_face<1>(c.n, c.u, Pl, r0.x, ur, Pr, Py, EFy);
+        const double Pr[3] = {S.pxy[tn], y2.x, y2.y};
+        bme_face<1>(c.n, c.u, Pl, y0.x, ur, Pr, Py, EFy);
         double* fy = S.fy;
         sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
         sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
         fy[4 * PP + t] = EFy[5];
     }
     if (f.star_row) {
-        const int tr = f.tx < FX - 1 ? t + 1 : t;
-        const double2 r0 = lds2(S.nu + 2 * tr), r1 = lds2(S.uu + 2 * tr), r2 = lds2(S.px + 2 * tr);
-        const double ur[3] = {r0.y, r1.x, r1.y};
+        const int te = f.tx < FX - 1 ? t + 1 : t;
+        const double2 x0 = lds2(S.nu + 2 * te), x1 = lds2(S.uu + 2 * te), x2 = lds2(S.px + 2 * te);
+        const double ur[3] = {x0.y, x1.x, x1.y};
         const double Pl[3] = {c.Pi[0], c.Pi[1], c.Pi[2]};
-        const double Pr[3] = {r2.x, S.pxy[tr], r2.y};
+        const double Pr[3] = {x2.x, S.pxy[te], x2.y};
         double Px[3], EFx[6];
-        bme_face<0>(c.n, c.u, Pl, r0.x, ur, Pr, Px, EFx);
+        bme_face<0>(c.n, c.u, Pl, x0.x, ur, Pr, Px, EFx);
 #pragma unroll
-        for (int q = 0; q < 3; ++q) c.acc[q] -= th * (Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1));
+        for (int q = 0; q < 3; ++q) c.acc[q] -= th2 * (Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1));
 #pragma unroll
-        for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th * (EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1));
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th4 * (EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1));
         gx = (S.phi[t + 1] - S.phi[t - 1]) * inv2h;
         gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
     }
@@ -609,9 +640,9 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
         const double* fy = S.fy + 2 * (t - FX);
         const double2 l0 = lds2(fy), l1 = lds2(fy + PP), l2 = lds2(fy + 2 * PP), l3 = lds2(fy + 3 * PP);
         const double l4 = S.fy[4 * PP + t - FX];
-        c.acc[0] -= th * (Py[0] - l0.x); c.acc[1] -= th * (Py[1] - l0.y); c.acc[2] -= th * (Py[2] - l1.x);
-        c.acc[3] -= th * (EFy[0] - l1.y); c.acc[4] -= th * (EFy[1] - l2.x); c.acc[5] -= th * (EFy[2] - l2.y);
-        c.acc[6] -= th * (EFy[3] - l3.x); c.acc[7] -= th * (EFy[4] - l3.y); c.acc[8] -= th * (EFy[5] - l4);
+        c.acc[0] -= th2 * (Py[0] - l0.x); c.acc[1] -= th2 * (Py[1] - l0.y); c.acc[2] -= th2 * (Py[2] - l1.x);
+        c.acc[3] -= th4 * (EFy[0] - l1.y); c.acc[4] -= th4 * (EFy[1] - l2.x); c.acc[5] -= th4 * (EFy[2] - l2.y);
+        c.acc[6] -= th4 * (EFy[3] - l3.x); c.acc[7] -= th4 * (EFy[4] - l3.y); c.acc[8] -= th4 * (EFy[5] - l4);
         // gravity (reading G5): -tau n g_i and -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
         const double gr[3] = {gx, gy, (c.phin - c.phim) * inv2h};
         double uc[3];
@@ -659,9 +690,9 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
         } else {
             o[0] = c.n;
 #pragma unroll
-            for (int d = 0; d < 3; ++d) o[1 + d] = fma(-th, Pz[d], c.acc[d]) * c.in;
+            for (int d = 0; d < 3; ++d) o[1 + d] = fma(-th2, Pz[d], c.acc[d]) * c.in;
 #pragma unroll
-            for (int q = 0; q < 6; ++q) o[4 + q] = fma(-th, EFz[q], c.acc[3 + q]);
+            for (int q = 0; q < 6; ++q) o[4 + q] = fma(-th4, EFz[q], c.acc[3 + q]);
         }
         sts2(rs + 2 * t, o[0], o[3]); sts2(rs + PP + 2 * t, o[1], o[2]); sts2(rs + 2 * PP + 2 * t, o[4], o[5]);
         sts2(rs + 3 * PP + 2 * t, o[6], o[7]); sts2(rs + 4 * PP + 2 * t, o[8], o[9]);
@@ -670,18 +701,18 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
             sts2(rg + 2 * t, o[0], o[3]); sts2(rg + PP + 2 * t, o[1], o[2]); sts2(rg + 2 * PP + 2 * t, o[4], o[5]);
             sts2(rg + 3 * PP + 2 * t, o[6], o[7]); sts2(rg + 4 * PP + 2 * t, o[8], o[9]);
         }
-        if (do_out) {                         // z-average of w*_x, w*_y for plane j-1
+        if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
             const double2 wm = lds2(S.ring + ring_slot(j - 2) * BME_SLOT + PP + 2 * t);
             const double2 w0 = lds2(S.ring + ring_slot(j - 1) * BME_SLOT + PP + 2 * t);
-            sts2(S.tz + 2 * t, avg3(wm.x, w0.x, o[1]), avg3(wm.y, w0.y, o[2]));
+            sts2(S.tz + 2 * t, sum3(wm.x, w0.x, o[1]), sum3(wm.y, w0.y, o[2]));
         }
     }
     sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
     sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1]; S.phi[t] = c.phin;
 #pragma unroll
-    for (int d = 0; d < 3; ++d) c.acc[d] = fma(th, Pz[d], Un[1 + d]);
+    for (int d = 0; d < 3; ++d) c.acc[d] = fma(th2, Pz[d], Un[1 + d]);
 #pragma unroll
-    for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(th, EFz[q], Un[4 + q]);
+    for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(th4, EFz[q], Un[4 + q]);
     c.n = n_n; c.in = in_n;
 #pragma unroll
     for (int d = 0; d < 3; ++d) c.u[d] = u_n[d];
@@ -706,19 +737,17 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
 
     // D: Lagrangian stage of plane j-1 (ring planes j-2, j-1, j)
     if (f.out_row) {
-        const double* rp = rs;
-        const double Sz_new = avg9_wz(rp, t);
+        const double Sz_new = sum9_wz(rs, t);             // 16 x
         if (bot_dup) c.Sz_prev = Sz_new;
         if (do_wzp) {
-            const double wzp = 0.5 * (c.Sz_prev + Sz_new);
+            const double wzp = c.Sz_prev + Sz_new;        // 32 x face velocity between planes j-1 and j
             if (do_out) {
-                const double* r0 = S.ring + ring_slot(j - 1) * BME_SLOT;
-                const double* rm = S.ring + ring_slot(j - 2) * BME_SLOT;
                 double wxm, wxp, wym, wyp;
                 face_vel_xy(S.tz, t, wxm, wxp, wym, wyp);
-                const LagCoef lc = lag_coef(th, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
+                const LagCoef lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
                 double out[NBME];
-                lagrange_cell<6>(rm, r0, rp, t, lc, out);
+                lagrange_lower<6>(S.ring + ring_slot(j - 2) * BME_SLOT, t, lc, out);
+                lagrange_rest<6>(S.ring + ring_slot(j - 1) * BME_SLOT, rs, t, lc, out);
                 if (f.is_out) {
                     const size_t off = f.base + (size_t)(j - 1) * f.nxny;
 #pragma unroll
@@ -732,9 +761,9 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
                         const double ud = out[1 + d] * inn;
                         const double Pdd = fma(-out[1 + d], ud, out[dd[d]]);
                         const double c2 = 3.0 * Pdd * inn;
-                        const double s = fabs(ud) + c2 * frsqrt(c2);
-                        if (!(Pdd > 0.0) || !(s <= 1.7976931348623157e308)) c.bad = 1;
-                        c.smax = fmax(c.smax, s);
+                        const double sp = fabs(ud) + c2 * frsqrt(c2);
+                        if (!(Pdd > 0.0) || !(sp <= 1.7976931348623157e308)) c.bad = 1;
+                        c.smax = fmax(c.smax, sp);
                     }
                 }
             }
@@ -750,6 +779,10 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
 #pragma unroll
         for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
         c.phin = phi_load(pc, j + 2, zm, g.nz);
+        // pull plane j+3 into L2 so that the next staging is an L2 hit
+        const size_t off3 = f.base + (size_t)map_safe(j + 3, g.nz, g.bcz) * f.nxny;
+#pragma unroll
+        for (int q = 0; q < NBME; ++q) prefetch_l2(a.U[q] + off3);
     }
     cp_async_commit();
 }
@@ -796,9 +829,9 @@ k_fused_bme(FusedArgs<NBME> a) {
         double Pz[3], EFz[6];
         bme_face<2>(n_a, u_a, Pz_a, c.n, c.u, Pr, Pz, EFz);
 #pragma unroll
-        for (int d = 0; d < 3; ++d) c.acc[d] = fma(th, Pz[d], U0[1 + d]);
+        for (int d = 0; d < 3; ++d) c.acc[d] = fma(0.5 * th, Pz[d], U0[1 + d]);
 #pragma unroll
-        for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(th, EFz[q], U0[4 + q]);
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(0.25 * th, EFz[q], U0[4 + q]);
         sts2(S.nu + 2 * t, c.n, c.u[0]); sts2(S.uu + 2 * t, c.u[1], c.u[2]); sts2(S.px + 2 * t, c.Pi[0], c.Pi[2]);
         sts2(S.py + 2 * t, c.Pi[3], c.Pi[4]); S.pxy[t] = c.Pi[1]; S.phi[t] = c.phi0;
         // stage plane z0 where U*(z0-1) will be written
