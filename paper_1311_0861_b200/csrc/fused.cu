@@ -166,13 +166,22 @@ __device__ __forceinline__ double sum3(double a, double b, double c) { return fm
 // so that every neighbour access is one 128-bit load.
 constexpr int PP = 2 * PL;   // doubles per pair plane
 
-// 16 x the 3x3 (omega x omega) average of the second member of pair plane P0 (w*_z) around cell t
+// Values of the x neighbours come from the adjacent lanes (a footprint row is one warp): a
+// shuffle costs about a quarter of the shared-memory wavefronts of the load it replaces.  Lanes
+// 0 and 31 get their own value back; they are halo columns whose results are never used.
+constexpr unsigned FULL = 0xffffffffu;
+__device__ __forceinline__ double from_left(double v) { return __shfl_up_sync(FULL, v, 1); }
+__device__ __forceinline__ double from_right(double v) { return __shfl_down_sync(FULL, v, 1); }
+__device__ __forceinline__ double2 from_left(double2 v) { return make_double2(from_left(v.x), from_left(v.y)); }
+__device__ __forceinline__ double2 from_right(double2 v) { return make_double2(from_right(v.x), from_right(v.y)); }
+// 4 x the (1/4,1/2,1/4) average along x of a per-thread value
+__device__ __forceinline__ double sum3_x(double v) { return sum3(from_left(v), v, from_right(v)); }
+
+// 16 x the 3x3 (omega x omega) average of the second member of pair plane P0 (w*_z) around cell t.
+// Must be called by whole warps.
 __device__ __forceinline__ double sum9_wz(const double* __restrict__ r, int t) {
-    const double* s = r + 1;
-    const double lo = sum3(s[2 * (t - FX - 1)], s[2 * (t - FX)], s[2 * (t - FX + 1)]);
-    const double mi = sum3(s[2 * (t - 1)], s[2 * t], s[2 * (t + 1)]);
-    const double hi = sum3(s[2 * (t + FX - 1)], s[2 * (t + FX)], s[2 * (t + FX + 1)]);
-    return sum3(lo, mi, hi);
+    const double2 lo = lds2(r + 2 * (t - FX)), mi = lds2(r + 2 * t), hi = lds2(r + 2 * (t + FX));
+    return sum3(sum3_x(lo.y), sum3_x(mi.y), sum3_x(hi.y));
 }
 
 // Upwind flux form of one cell in coefficient form:
@@ -216,17 +225,18 @@ __device__ __forceinline__ void lagrange_lower(const double* __restrict__ rm, in
 template <int NO>
 __device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, const double* __restrict__ rp, int t,
                                               const LagCoef& c, double out[4 + NO]) {
-    const double2 a0 = lds2(r0 + 2 * t), axm = lds2(r0 + 2 * (t - 1)), axp = lds2(r0 + 2 * (t + 1));
-    const double2 aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
+    // whole warps only: the x neighbours are fetched by shuffle
+    const double2 a0 = lds2(r0 + 2 * t), aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
     const double2 azp = lds2(rp + 2 * t);
+    const double2 axm = from_left(a0), axp = from_right(a0);
     const double d0 = c.c0 * a0.x, dxm = c.xm * axm.x, dxp = c.xp * axp.x, dym = c.ym * aym.x, dyp = c.yp * ayp.x,
                  dzp = c.zp * azp.x;
     out[0] = ((out[0] + d0) + (dxm + dxp)) + ((dym + dyp) + dzp);
     out[3] = fma(dzp, azp.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, fma(d0, a0.y, out[3]))))));
     {
-        const double2 b0 = lds2(r0 + PP + 2 * t), bxm = lds2(r0 + PP + 2 * (t - 1)), bxp = lds2(r0 + PP + 2 * (t + 1));
-        const double2 bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
+        const double2 b0 = lds2(r0 + PP + 2 * t), bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
         const double2 bzp = lds2(rp + PP + 2 * t);
+        const double2 bxm = from_left(b0), bxp = from_right(b0);
         out[1] = fma(dzp, bzp.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, fma(d0, b0.x, out[1]))))));
         out[2] = fma(dzp, bzp.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, fma(d0, b0.y, out[2]))))));
     }
@@ -234,15 +244,15 @@ __device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, con
     for (int P = 0; P < (NO + 1) / 2; ++P) {
         const int o = (2 + P) * PP;
         if (2 * P + 1 < NO) {
-            const double2 e0 = lds2(r0 + o + 2 * t), exm = lds2(r0 + o + 2 * (t - 1)), exp_ = lds2(r0 + o + 2 * (t + 1));
-            const double2 eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
+            const double2 e0 = lds2(r0 + o + 2 * t), eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
             const double2 ezp = lds2(rp + o + 2 * t);
+            const double2 exm = from_left(e0), exp_ = from_right(e0);
             out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, fma(c.c0, e0.x, out[4 + 2 * P]))))));
             out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, fma(c.c0, e0.y, out[5 + 2 * P]))))));
         } else {
-            const double e0 = r0[o + 2 * t], exm = r0[o + 2 * (t - 1)], exp_ = r0[o + 2 * (t + 1)];
-            const double eym = r0[o + 2 * (t - FX)], eyp = r0[o + 2 * (t + FX)];
+            const double e0 = r0[o + 2 * t], eym = r0[o + 2 * (t - FX)], eyp = r0[o + 2 * (t + FX)];
             const double ezp = rp[o + 2 * t];
+            const double exm = from_left(e0), exp_ = from_right(e0);
             out[4 + 2 * P] = fma(c.zp, ezp, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, fma(c.c0, e0, out[4 + 2 * P]))))));
         }
     }
@@ -252,11 +262,11 @@ __device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, con
 // w*_y pair plane (s_tz): x faces = sum of the y-summed columns tx-1|tx and tx|tx+1, y faces likewise.
 __device__ __forceinline__ void face_vel_xy(const double* __restrict__ s_tz, int t, double& wxm, double& wxp, double& wym,
                                             double& wyp) {
-    const double2 mm = lds2(s_tz + 2 * (t - FX - 1)), m0 = lds2(s_tz + 2 * (t - FX)), mp = lds2(s_tz + 2 * (t - FX + 1));
-    const double2 zm = lds2(s_tz + 2 * (t - 1)), z0 = lds2(s_tz + 2 * t), zp = lds2(s_tz + 2 * (t + 1));
-    const double2 pm = lds2(s_tz + 2 * (t + FX - 1)), p0 = lds2(s_tz + 2 * (t + FX)), pp = lds2(s_tz + 2 * (t + FX + 1));
-    const double a_m = sum3(mm.x, zm.x, pm.x), a_0 = sum3(m0.x, z0.x, p0.x), a_p = sum3(mp.x, zp.x, pp.x);
-    const double b_m = sum3(mm.y, m0.y, mp.y), b_0 = sum3(zm.y, z0.y, zp.y), b_p = sum3(pm.y, p0.y, pp.y);
+    // whole warps only (shuffles)
+    const double2 m0 = lds2(s_tz + 2 * (t - FX)), z0 = lds2(s_tz + 2 * t), p0 = lds2(s_tz + 2 * (t + FX));
+    const double a_0 = sum3(m0.x, z0.x, p0.x);
+    const double a_m = from_left(a_0), a_p = from_right(a_0);
+    const double b_m = sum3_x(m0.y), b_0 = sum3_x(z0.y), b_p = sum3_x(p0.y);
     wxm = a_m + a_0; wxp = a_0 + a_p;
     wym = b_m + b_0; wyp = b_0 + b_p;
 }
@@ -573,10 +583,10 @@ k_fused_gas(FusedArgs<NGAS> a) {
 // Collisionless component: fields n, nu (3), nE_ij (6: xx xy xz yy yz zz).
 // Shared planes (of PL doubles): primitives (n,ux) (uy,uz) (Pxx,Pxz) (Pyy,Pyz) pairs 8 + Pxy 1 +
 // Phi 1, y-flux (Ps0,Ps1) (Ps2,EF0) (EF1,EF2) (EF3,EF4) pairs 8 + EF5 1, ring 3 x 5 pair planes = 30,
-// z-averaged (w*_x,w*_y) pair 2  ->  51 planes = 204 KB.
+// z-averaged (w*_x,w*_y) pair 2, staged Phi 1  ->  52 planes = 208 KB.
 // =================================================================================================
 constexpr int BME_SLOT = 5 * PP;
-constexpr int BME_PLANES = 10 + 9 + 3 * 10 + 2;
+constexpr int BME_PLANES = 10 + 9 + 3 * 10 + 2 + 1;
 
 struct BmeCarry {
     double n, in, u[3], Pi[6];            // primitives of the current plane j (own cell)
@@ -587,7 +597,7 @@ struct BmeCarry {
 };
 
 struct BmeShared {
-    double *nu, *uu, *px, *py, *pxy, *phi, *fy, *ring, *tz;
+    double *nu, *uu, *px, *py, *pxy, *phi, *fy, *ring, *tz, *phst;
 };
 
 template <bool ST>
@@ -669,6 +679,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
         Un[0] = s0.x; Un[1] = s0.y; Un[2] = s1.x; Un[3] = s1.y; Un[4] = s2.x; Un[5] = s2.y;
         Un[6] = s3.x; Un[7] = s3.y; Un[8] = s4.x; Un[9] = s4.y;
     }
+    const double phi_n2 = S.phst[t];      // Phi(j+2), staged with plane j+1
     const double n_n = Un[0];
     const double in_n = frcp(n_n);
     const double u_n[3] = {Un[1] * in_n, Un[2] * in_n, Un[3] * in_n};
@@ -718,7 +729,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
     for (int d = 0; d < 3; ++d) c.u[d] = u_n[d];
 #pragma unroll
     for (int q = 0; q < 6; ++q) c.Pi[q] = Pi_n[q];
-    c.phim = c.phi0; c.phi0 = c.phin;
+    c.phim = c.phi0; c.phi0 = c.phin; c.phin = phi_n2;
     __syncthreads();
 
     if (f.block_fix) {
@@ -771,14 +782,14 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
         }
         c.Sz_prev = Sz_new;
     }
-    // stage plane j+2 into the slot D just finished with (own column only); Phi(j+2) to a register
+    // stage plane j+2 into the slot D just finished with (own column only), and Phi(j+3)
     if (stage_next) {
         const int zm = map_safe(j + 2, g.nz, g.bcz);
         const size_t off = f.base + (size_t)zm * f.nxny;
         double* st = S.ring + ring_slot(j + 1) * BME_SLOT + 2 * t;
 #pragma unroll
         for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
-        c.phin = phi_load(pc, j + 2, zm, g.nz);
+        cp_async8(S.phst + t, phi_ptr(pc, j + 3, map_safe(j + 3, g.nz, g.bcz), g.nz));
         // pull plane j+3 into L2 so that the next staging is an L2 hit
         const size_t off3 = f.base + (size_t)map_safe(j + 3, g.nz, g.bcz) * f.nxny;
 #pragma unroll
@@ -793,7 +804,7 @@ k_fused_bme(FusedArgs<NBME> a) {
     double* sm = reinterpret_cast<double*>(sm2);
     BmeShared S;
     S.nu = sm; S.uu = sm + 2 * PL; S.px = sm + 4 * PL; S.py = sm + 6 * PL; S.pxy = sm + 8 * PL; S.phi = sm + 9 * PL;
-    S.fy = sm + 10 * PL; S.ring = sm + 19 * PL; S.tz = S.ring + 3 * BME_SLOT;
+    S.fy = sm + 10 * PL; S.ring = sm + 19 * PL; S.tz = S.ring + 3 * BME_SLOT; S.phst = S.tz + 2 * PL;
 
     const Geo& g = a.g;
     const Foot f = make_foot(g, a.zchunk);
@@ -841,6 +852,7 @@ k_fused_bme(FusedArgs<NBME> a) {
 #pragma unroll
         for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
         c.phin = phi_load(pc, f.z0, zm, g.nz);
+        cp_async8(S.phst + t, phi_ptr(pc, f.z0 + 1, map_safe(f.z0 + 1, g.nz, g.bcz), g.nz));
         cp_async_commit();
     }
     __syncthreads();
@@ -857,14 +869,20 @@ k_fused_bme(FusedArgs<NBME> a) {
 // launches
 // -------------------------------------------------------------------------------------------------
 static int pick_zchunk(const gp_ctx* c, int tiles_xy) {
-    // enough blocks for >= 8 waves of 148 one-block SMs, chunks no shorter than 16 planes
+    // One block per SM: the grid runs in waves of 148 blocks, and every chunk pays about three
+    // planes of pipeline fill.  Pick the chunk length that minimises waves x (planes + fill).
     const int nz = c->g.nz;
-    int chunks = (8 * 148 + tiles_xy - 1) / tiles_xy;
-    if (chunks < 1) chunks = 1;
-    int zc = (nz + chunks - 1) / chunks;
-    if (zc < 16) zc = 16;
-    if (zc > nz) zc = nz;
-    return zc;
+    int best = nz;
+    long long best_cost = -1;
+    for (int chunks = 1; chunks <= 64; ++chunks) {
+        const int zc = (nz + chunks - 1) / chunks;
+        if (zc < 16 && chunks > 1) break;
+        const long long blocks = (long long)tiles_xy * ((nz + zc - 1) / zc);
+        const long long waves = (blocks + 147) / 148;
+        const long long cost = waves * (zc + 3);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = zc; }
+    }
+    return best;
 }
 
 template <int NF, class K>
