@@ -44,6 +44,7 @@ ALGO_BYTES_PER_CELL = {
     "cfl": 15 * W,                          # a-6
     "poisson_source": 3 * W,
     "poisson_green": 2 * W,                 # half spectrum, complex: read + write (nx/2+1)/nx * 16 B each
+    "poisson_zpass_green": 2 * W,           # fused z transform + Green + inverse: the half spectrum once each way
 }
 # minimum bytes per cell per FULL step for the headline roofline fraction
 STEP_BYTES_PER_CELL = {("gas",): 80, ("gas", "isolated"): 304, ("gas", "stars", "periodic"): 336,

@@ -22,7 +22,7 @@ static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 static const char* const kKernelNames[K_NUM] = {
     "eulerian_gas", "lagrangian_gas", "eulerian_bme", "lagrangian_bme", "cfl", "poisson_source", "cufft_forward",
     "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract",
-    "hydro_gas_fused", "hydro_bme_fused"};
+    "hydro_gas_fused", "hydro_bme_fused", "poisson_zpass_green"};
 
 void tic(gp_ctx* c, int kid) {
     Timing* t = c->tim;
@@ -125,11 +125,14 @@ static int ensure_storage(gp_ctx* c) {
     c->d_flag_next = (int*)(small + 192);
     c->cfl_cached = false;
     c->spec = nullptr; c->padded = nullptr; c->kspec = nullptr; c->tabx = c->taby = c->tabz = nullptr;
+    c->ztw = nullptr; c->src = nullptr; c->src_cached = false;
     if (g.poisson == GP_POISSON_PERIODIC) {
         c->spec = (cufftDoubleComplex*)take(((size_t)g.nx / 2 + 1) * g.ny * g.nz * sizeof(cufftDoubleComplex));
         c->tabx = (double*)take(((size_t)g.nx + g.ny + g.nz) * sizeof(double));
         c->taby = c->tabx + g.nx;
         c->tabz = c->taby + g.ny;
+        c->ztw = (double*)take(2 * (size_t)g.nz * sizeof(double));
+        if ((g.components & GP_GAS) && (g.components & GP_STARS)) c->src = (double*)take(N * sizeof(double));
     } else if (g.poisson == GP_POISSON_ISOLATED) {
         const size_t half = ((size_t)g.nx + 1) * (2 * (size_t)g.ny) * (2 * (size_t)g.nz);
         c->spec = (cufftDoubleComplex*)take(half * sizeof(cufftDoubleComplex));
@@ -286,6 +289,7 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));   // the host buffer may be reused on return
     if (field == GP_PHI) return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
     c->cfl_cached = false;
+    c->src_cached = false;
     return GP_OK;
 }
 
@@ -334,13 +338,18 @@ int gp_step(gp_ctx* c, double dt) {
     if (rc != GP_OK) return rc;
     const double* d_dt = dt > 0.0 ? nullptr : c->d_dt;
     if ((rc = launch_cfl_reset_next(c)) != GP_OK) return rc;
-    if (c->g.components & GP_GAS) {
-        if ((rc = launch_fused_gas(c, dt, d_dt)) != GP_OK) return rc;
-        for (int f = 0; f < NGAS; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
-    }
+    // With both components and the periodic solve, the source rho + n of the next solve rides in
+    // the epilogue of the gas kernel, which therefore runs second (n is then already new).
+    c->src_cached = false;
     if (c->g.components & GP_STARS) {
         if ((rc = launch_fused_bme(c, dt, d_dt)) != GP_OK) return rc;
         for (int f = NGAS; f < NHYD; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
+    }
+    if (c->g.components & GP_GAS) {
+        double* src_out = c->src;          // non-null only with both components and the periodic solve
+        if ((rc = launch_fused_gas(c, dt, d_dt, src_out ? c->U[GP_N] : nullptr, src_out)) != GP_OK) return rc;
+        for (int f = 0; f < NGAS; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
+        c->src_cached = src_out != nullptr;
     }
     c->cfl_cached = true;
     return GP_OK;

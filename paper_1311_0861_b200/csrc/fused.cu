@@ -282,6 +282,8 @@ struct FusedArgs {
     int zchunk;
     unsigned long long* smax_bits;
     int* flag;
+    const double* src_in;     // gas kernel only: density n of the new collisionless state, or null
+    double* src_out;          // ... and where to write the Poisson source rho + n of the new state, or null
 };
 
 struct Foot {
@@ -476,6 +478,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
     // first (own column only) and then handed to the staging of plane j+2.
     double out[NGAS];
     LagCoef lc;
+    double n_other = 0.0;
     bool emit = false;
     if (f.out_row) {
         const double Sz_new = sum9_wz(rs, t);             // 16 x
@@ -486,6 +489,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
                 double wxm, wxp, wym, wyp;
                 face_vel_xy(S.tz, t, wxm, wxp, wym, wyp);
                 lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
+                // density of the other component for the Poisson source: asked for early, used last
+                if (a.src_in && f.is_out) n_other = a.src_in[f.base + (size_t)(j - 1) * f.nxny];
                 lagrange_lower<1>(S.ring + ring_slot(j - 2) * GAS_SLOT, t, lc, out);
                 emit = true;
             }
@@ -509,6 +514,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
             const size_t off = f.base + (size_t)(j - 1) * f.nxny;
 #pragma unroll
             for (int q = 0; q < NGAS; ++q) a.Un[q][off] = out[q];
+            if (a.src_out) a.src_out[off] = out[0] + n_other;
             // CFL of the new state (reading G4)
             const double irn = frcp(out[0]);
             const double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
@@ -886,8 +892,10 @@ static int pick_zchunk(const gp_ctx* c, int tiles_xy) {
 }
 
 template <int NF, class K>
-static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, double dt, const double* d_dt) {
+static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, double dt, const double* d_dt,
+                          const double* src_in = nullptr, double* src_out = nullptr) {
     FusedArgs<NF> a;
+    a.src_in = src_in; a.src_out = src_out;
     a.g = Geo{c->g.nx, c->g.ny, c->g.nz, c->bc.x, c->bc.y, c->bc.z};
     for (int f = 0; f < NF; ++f) { a.U[f] = c->U[f0 + f]; a.Un[f] = c->Us[f0 + f]; }
     a.phi = Phi{c->phi, c->phig[0], c->phig[1], c->phig[2], c->phig[3], c->phig[4], c->phig[5]};
@@ -910,8 +918,8 @@ static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, doub
     return GP_OK;
 }
 
-int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt) {
-    return launch_fused_t<NGAS>(c, k_fused_gas, 0, GAS_PLANES, K_FUSED_GAS, dt, d_dt);
+int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out) {
+    return launch_fused_t<NGAS>(c, k_fused_gas, 0, GAS_PLANES, K_FUSED_GAS, dt, d_dt, src_in, src_out);
 }
 
 int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt) {

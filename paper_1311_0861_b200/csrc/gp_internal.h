@@ -45,7 +45,7 @@ void set_error(const char* fmt, ...);
 
 // Kernels (and cuFFT executions) that can be timed one by one with CUDA events.
 enum KernelId { K_EUL_GAS = 0, K_LAG_GAS, K_EUL_BME, K_LAG_BME, K_CFL, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV,
-                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_FUSED_GAS, K_FUSED_BME, K_NUM };
+                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_NUM };
 
 struct Timing {
     bool on = false;
@@ -88,6 +88,10 @@ struct gp_ctx {
     double* padded;                 // isolated: (2nx)(2ny)(2nz) real array
     double* kspec;                  // isolated: real spectrum of the 1/r kernel
     double* tabx; double* taby; double* tabz;   // periodic: 1 - (2/3) sin^2(pi k/N) per axis
+    double* ztw;                    // periodic, fused z pass: exp(-2 pi i k/nz), nz complex values
+    bool zfused;                    // periodic: 2-D batched cuFFT plans + the fused z pass (zpass.cu)
+    double* src;                    // periodic, gas + stars: rho + n assembled here (by the fused step or k_source)
+    bool src_cached;                // src holds rho + n of the current state (written by the fused step)
 
     long long n_own, n_fft;
     gp::Timing* tim;
@@ -106,7 +110,8 @@ int launch_cfl_reset_next(gp_ctx* c);
 int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz);
 
 // fused.cu
-int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt);
+// src_out != nullptr: also write rho + n of the new state there (src_in = the new n, or nullptr)
+int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out);
 int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt);
 int math_selftest(int n, const double* x, double* rcp, double* rsq);
 
@@ -115,6 +120,10 @@ int poisson_setup(gp_ctx* c);
 void poisson_teardown(gp_ctx* c);
 int poisson_solve(gp_ctx* c);
 size_t poisson_storage_bytes(const gp_grid* g);
+
+// zpass.cu
+bool zpass_supported(int nz);
+int launch_zpass(gp_ctx* c, double coef6);
 
 }  // namespace gp
 

@@ -19,7 +19,10 @@ static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 size_t poisson_storage_bytes(const gp_grid* g) {
     const size_t nx = g->nx, ny = g->ny, nz = g->nz;
     if (g->poisson == GP_POISSON_PERIODIC) {
-        return align256((nx / 2 + 1) * ny * nz * sizeof(cufftDoubleComplex)) + 3 * align256((nx + ny + nz) * sizeof(double));
+        size_t b = align256((nx / 2 + 1) * ny * nz * sizeof(cufftDoubleComplex)) + 3 * align256((nx + ny + nz) * sizeof(double));
+        b += align256(2 * nz * sizeof(double));                                   // twiddles of the fused z pass
+        if ((g->components & GP_GAS) && (g->components & GP_STARS)) b += align256(nx * ny * nz * sizeof(double));   // rho + n
+        return b;
     }
     if (g->poisson == GP_POISSON_ISOLATED) {
         const size_t half = (nx + 1) * (2 * ny) * (2 * nz);
@@ -133,8 +136,24 @@ int poisson_setup(gp_ctx* c) {
     if (c->fft_ready) return GP_OK;
     const int nx = c->g.nx, ny = c->g.ny, nz = c->g.nz;
     if (c->g.poisson == GP_POISSON_PERIODIC) {
-        GP_CUFFT(cufftPlan3d(&c->plan_fwd, nz, ny, nx, CUFFT_D2Z));
-        GP_CUFFT(cufftPlan3d(&c->plan_inv, nz, ny, nx, CUFFT_Z2D));
+        c->zfused = zpass_supported(nz);
+        if (c->zfused) {
+            // batched 2-D real transforms over the xy planes; the z direction is zpass.cu's
+            int n[2] = {ny, nx}, rembed[2] = {ny, nx}, cembed[2] = {ny, nx / 2 + 1};
+            GP_CUFFT(cufftPlanMany(&c->plan_fwd, 2, n, rembed, 1, ny * nx, cembed, 1, ny * (nx / 2 + 1), CUFFT_D2Z, nz));
+            GP_CUFFT(cufftPlanMany(&c->plan_inv, 2, n, cembed, 1, ny * (nx / 2 + 1), rembed, 1, ny * nx, CUFFT_Z2D, nz));
+            std::vector<double> w(2 * (size_t)nz);
+            for (int k = 0; k < nz; ++k) {
+                const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)nz;
+                w[2 * k] = (double)cosl(a);
+                w[2 * k + 1] = (double)-sinl(a);
+            }
+            GP_CUDA(cudaMemcpyAsync(c->ztw, w.data(), w.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+            GP_CUDA(cudaStreamSynchronize(c->stream));
+        } else {
+            GP_CUFFT(cufftPlan3d(&c->plan_fwd, nz, ny, nx, CUFFT_D2Z));
+            GP_CUFFT(cufftPlan3d(&c->plan_inv, nz, ny, nx, CUFFT_Z2D));
+        }
         const double pi = 3.14159265358979323846;
         std::vector<double> t((size_t)nx + ny + nz);
         for (int k = 0; k < nx; ++k) { const double s = std::sin(pi * k / nx); t[k] = 1.0 - 2.0 / 3.0 * s * s; }
@@ -183,20 +202,33 @@ int poisson_solve(gp_ctx* c) {
     const double pi = 3.14159265358979323846;
     if (c->g.poisson == GP_POISSON_PERIODIC) {
         const size_t half = ((size_t)nx / 2 + 1) * ny * nz;
-        tic(c, K_SOURCE);
-        k_source<<<blocks_for(c->N), 256, 0, c->stream>>>(c->N, rho, n, c->phi);
-        toc(c);
+        // source rho + n: one component -> its density is transformed in place of a
+        // copy; both -> c->src, already written by the fused step unless the state was set since
+        const double* s = rho && n ? c->src : (rho ? rho : n);
+        if (rho && n && !c->src_cached) {
+            tic(c, K_SOURCE);
+            k_source<<<blocks_for(c->N), 256, 0, c->stream>>>(c->N, rho, n, c->src);
+            toc(c);
+            c->n_own += 1;
+        }
         tic(c, K_FFT_FWD);
-        GP_CUFFT(cufftExecD2Z(c->plan_fwd, c->phi, c->spec));
+        GP_CUFFT(cufftExecD2Z(c->plan_fwd, const_cast<double*>(s), c->spec));
         toc(c);
         const double coef = -4.0 * pi * c->g.G * c->g.h * c->g.h / (double)c->N;
-        tic(c, K_GREEN);
-        k_green_periodic<<<blocks_for(half), 256, 0, c->stream>>>(nx / 2 + 1, ny, nz, c->tabx, c->taby, c->tabz, coef, c->spec);
-        toc(c);
+        if (c->zfused) {
+            tic(c, K_ZPASS);
+            rc = launch_zpass(c, coef / 6.0);
+            toc(c);
+            if (rc != GP_OK) return rc;
+        } else {
+            tic(c, K_GREEN);
+            k_green_periodic<<<blocks_for(half), 256, 0, c->stream>>>(nx / 2 + 1, ny, nz, c->tabx, c->taby, c->tabz, coef, c->spec);
+            toc(c);
+        }
         tic(c, K_FFT_INV);
         GP_CUFFT(cufftExecZ2D(c->plan_inv, c->spec, c->phi));
         toc(c);
-        c->n_own += 2; c->n_fft += 2;
+        c->n_own += 1; c->n_fft += 2;
         GP_CUDA(cudaGetLastError());
         return launch_phi_ghost_bc(c, GP_BC_PERIODIC, GP_BC_PERIODIC, GP_BC_PERIODIC);
     }
