@@ -127,26 +127,58 @@ class ClockSampler(threading.Thread):
         return out
 
 
-def make_workload(args):
+CONFIG_NOTES = {1: "Sod tube 128x4x4, gas, no gravity", 2: "smooth gas 256^3, periodic, no gravity",
+                3: "cold collapse 256^3, gas + isolated FFT gravity", 4: "one disk 256^3, gas + collisionless + {p} FFT gravity",
+                5: "gas + collisionless + {p} FFT gravity"}
+
+
+def make_workload(args, sample_n=None):
+    """The BASELINE.json config args.config at full size, or (sample_n) the same recipe on a smaller grid."""
     from paper_1311_0861_b200 import workloads as wl
     poisson = wl.POISSON_PERIODIC if args.poisson == "periodic" else wl.POISSON_ISOLATED
-    w = wl.two_disks(n=args.n, poisson=poisson)
-    name = f"two_disks_{args.n}^3 (BASELINE.json config 5: gas + collisionless + {args.poisson} FFT gravity)"
-    return w, name
+    c = args.config
+    if c == 5:
+        w = wl.two_disks(n=sample_n or args.n, poisson=poisson)
+    elif c == 4:
+        w = wl.disk(n=sample_n or 256, poisson=poisson)
+    elif c == 3:
+        w = wl.collapse(n=min(sample_n, 64) if sample_n else 256)
+    elif c == 2:
+        w = wl.smooth_gas(n=sample_n or 256)
+    else:
+        w = wl.sod()
+    return w, workload_name(args)
 
 
-def oracle_leg(sample_n, poisson, max_steps, budget_s):
-    """Time the CPU oracle, as it stands, on a bounded sample of the workload (same recipe at
-    sample_n^3, same cells per disk scale).  Returns (cells/s, threads, description, ms/step)."""
+def workload_name(args):
+    note = CONFIG_NOTES[args.config].format(p=args.poisson)
+    if args.config == 5:
+        return f"two_disks_{args.n}^3 (BASELINE.json config 5: {note})"
+    return f"{['', 'sod', 'smooth_gas', 'collapse', 'disk'][args.config]} (BASELINE.json config {args.config}: {note})"
+
+
+def step_bytes_key(w):
+    from paper_1311_0861_b200 import workloads as wl
+    key = (("gas",) if w.components & wl.GAS else ()) + (("stars",) if w.components & wl.STARS else ())
+    if w.poisson != wl.POISSON_NONE:
+        key += ("periodic" if w.poisson == wl.POISSON_PERIODIC else "isolated",)
+    return key
+
+
+def oracle_leg(args, max_steps, budget_s):
+    """Time the CPU oracle, as it stands, on a bounded sample of the workload (same recipe on an
+    args.ref_n^3 grid, same cells per disk scale).  Returns (cells/s, threads, description, ms/step)."""
     import oracle
     from paper_1311_0861_b200 import workloads as wl
-    w = wl.two_disks(n=sample_n, poisson=wl.POISSON_PERIODIC if poisson == "periodic" else wl.POISSON_ISOLATED)
+    w, _ = make_workload(args, sample_n=args.ref_n)
+    poisson = args.poisson if w.poisson != wl.POISSON_NONE else "no"
     o = oracle.Oracle(w.nx, w.ny, w.nz, w.h, w.components, w.poisson, w.G, w.gamma, w.bc)
     o.set_state(w.state())
     threads = oracle.get_threads()
 
     def step():
-        o.solve_poisson()
+        if w.poisson != wl.POISSON_NONE:
+            o.solve_poisson()
         o.step(o.max_dt(w.cfl))
 
     step()  # warm-up (page faults, kernel spectrum)
@@ -156,7 +188,7 @@ def oracle_leg(sample_n, poisson, max_steps, budget_s):
         step()
         n += 1
     dt = time.perf_counter() - t0
-    desc = (f"{n} full steps (max_dt + {poisson} Poisson + step) of the two_disks recipe at {sample_n}^3 "
+    desc = (f"{n} full steps (max_dt + {poisson} Poisson + step) of the {w.name} recipe on {w.nx}x{w.ny}x{w.nz} "
             f"({w.cells} cells), OpenMP on outer loops, {threads} threads")
     return w.cells * n / dt, threads, desc, 1e3 * dt / n
 
@@ -165,17 +197,17 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    _, wname = make_workload_name_only(args)
-    # each "step" is a bounded sample: one full oracle step at sample_n^3
+    wname = workload_name(args)
+    # each "step" is a bounded sample: one full oracle step of the same recipe on the args.ref_n grid
     import oracle
     from paper_1311_0861_b200 import workloads as wl
-    sample_n = args.ref_n
-    w = wl.two_disks(n=sample_n, poisson=wl.POISSON_PERIODIC if args.poisson == "periodic" else wl.POISSON_ISOLATED)
+    w, _ = make_workload(args, sample_n=args.ref_n)
     o = oracle.Oracle(w.nx, w.ny, w.nz, w.h, w.components, w.poisson, w.G, w.gamma, w.bc)
     o.set_state(w.state())
 
     def step():
-        o.solve_poisson()
+        if w.poisson != wl.POISSON_NONE:
+            o.solve_poisson()
         o.step(o.max_dt(w.cfl))
 
     for _ in range(args.warmup):
@@ -186,22 +218,18 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     value = w.cells * args.steps / dt
     threads = oracle.get_threads()
-    sample = (f"each step = one full oracle step of the same recipe at {sample_n}^3 ({w.cells} cells); "
+    sample = (f"each step = one full oracle step of the same recipe on {w.nx}x{w.ny}x{w.nz} ({w.cells} cells); "
               f"{args.steps} steps timed with perf_counter")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wname, "reference": "CPU oracle (oracle/, plain C++17) on host cores", "sample_grid": [sample_n] * 3},
+        "config": {"workload": wname, "reference": "CPU oracle (oracle/, plain C++17) on host cores", "sample_grid": [w.nx, w.ny, w.nz]},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
-
-
-def make_workload_name_only(args):
-    return None, f"two_disks_{args.n}^3 (BASELINE.json config 5: gas + collisionless + {args.poisson} FFT gravity)"
 
 
 def run_gpu(args):
@@ -231,9 +259,13 @@ def run_gpu(args):
     sim.synchronize()
     t_setup = time.perf_counter() - t_setup
 
+    from paper_1311_0861_b200 import workloads as wl
+    gravity = w.poisson != wl.POISSON_NONE
+
     def full_step():
         sim.max_dt(w.cfl, to_host=False)
-        sim.solve_poisson()
+        if gravity:
+            sim.solve_poisson()
         sim.step(0.0)
 
     for _ in range(args.warmup):
@@ -273,7 +305,8 @@ def run_gpu(args):
         for k in names:
             sim.set(k, host[k].numpy())            # H2D inside the timed region
         sim.max_dt(w.cfl)                          # dt comes back to the host
-        sim.solve_poisson()
+        if gravity:
+            sim.solve_poisson()
         sim.step(0.0)
         for k in names:
             sim.get(k, out=out[k].numpy())         # D2H of the step's result
@@ -300,12 +333,24 @@ def run_gpu(args):
     top = max(own, key=lambda k: own[k][0])
     top_ms = own[top][0] / own[top][1]
     algo = ALGO_BYTES_PER_CELL.get(top, 0) * cells
+    if not gravity and top.startswith("hydro_"):
+        algo -= W * cells                      # no Phi to read without gravity
     achieved = algo / (top_ms * 1e-3) / 1e9
-    wkey = f"two_disks_{args.n}_{args.poisson}"
+    wkey = f"{w.name}_{w.nx}_{args.poisson if gravity else 'nogravity'}"
     roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": stored_traffic(top, wkey), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": algo, "ms_per_launch": top_ms}
-    step_bytes = STEP_BYTES_PER_CELL[("gas", "stars", args.poisson)]
+    # the same kernel against the fp64 pipe: executed fp64 instructions of the committed
+    # ncu capture / the live duration, peak = 148 SMs x 64 lanes x max SM clock
+    roofline_alu = None
+    fp64_inst = (stored_traffic("fp64_warp_inst", wkey) or {}).get(top)
+    if fp64_inst:
+        peak_alu = 148 * 64 * (clocks.get("sm_max_mhz") or 1965) * 1e6 / 1e12
+        ach = fp64_inst * 32 / (top_ms * 1e-3) / 1e12
+        roofline_alu = {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak_alu,
+                        "unit": "T fp64 thread-instructions/s", "frac": ach / peak_alu,
+                        "peak_source": "148 SMs x 64 fp64 lanes (ncu pipe peak, DESIGN.md 8) x max SM clock"}
+    step_bytes = STEP_BYTES_PER_CELL[step_bytes_key(w)]
     per_gpu = value / world
     step_roofline = {"bytes_per_cell_step": step_bytes,
                      "frac_of_8TBs": per_gpu * step_bytes / 8.0e12,
@@ -314,22 +359,23 @@ def run_gpu(args):
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        v, threads, desc, _ = oracle_leg(args.ref_n, args.poisson, max_steps=20, budget_s=12.0)
+        v, threads, desc, _ = oracle_leg(args, max_steps=20, budget_s=12.0)
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": wname, "grid": [w.nx, w.ny, w.nz], "components": "gas+stars", "poisson": args.poisson,
+        "config": {"workload": wname, "grid": [w.nx, w.ny, w.nz], "components": "+".join(k for k in step_bytes_key(w) if k in ("gas", "stars")), "poisson": args.poisson if gravity else "none",
                    "cfl": w.cfl, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-                   "cache": f"inputs larger than L2: {len(names) * cells * W / 1e9:.1f} GB of state per step vs 126 MB L2 (no flush)",
+                   "cache": (f"inputs larger than L2: {len(names) * cells * W / 1e9:.1f} GB of state per step vs 126 MB L2 (no flush)"
+                             if len(names) * cells * W > 4 * 126e6 else "state fits in L2 (latency-bound case, not a bandwidth measurement)"),
                    "dt_after_run": dt_end, "setup_s": round(t_setup, 1)},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": bytes_dir, "d2h_bytes_per_step": bytes_dir,
                 "steps": e2e_steps, "ms_per_step": e2e_ms_max / e2e_steps},
         "gpu_launches": int(own1 - own0), "cufft_execs": int(fft1 - fft0),
-        "roofline": roofline, "step_roofline": step_roofline, "kernels": breakdown,
+        "roofline": roofline, "roofline_alu": roofline_alu, "step_roofline": step_roofline, "kernels": breakdown,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line), flush=True)
@@ -342,12 +388,16 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config (default 5, the headline); the others are parity cases timed for BASELINE.md")
     ap.add_argument("--n", type=int, default=512, help="grid size of the two-disk workload (BASELINE config 5: 512)")
     ap.add_argument("--poisson", default="periodic", choices=["periodic", "isolated"])
     ap.add_argument("--ref-n", type=int, default=128, help="grid size of the bounded sample the CPU oracle is timed on")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.config == 3:
+        args.poisson = "isolated"
     if args.warmup < 3:
         args.warmup = 3          # timing hygiene: at least three warm-up steps
     if args.impl == "reference":
