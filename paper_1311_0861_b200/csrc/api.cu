@@ -22,7 +22,8 @@ static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 static const char* const kKernelNames[K_NUM] = {
     "eulerian_gas", "lagrangian_gas", "eulerian_bme", "lagrangian_bme", "cfl", "poisson_source", "cufft_forward",
     "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract",
-    "hydro_gas_fused", "hydro_bme_fused", "poisson_zpass_green"};
+    "hydro_gas_fused", "hydro_bme_fused", "poisson_zpass_green", "poisson_iso_yfwd", "poisson_iso_zfused",
+    "poisson_iso_yinv"};
 
 void tic(gp_ctx* c, int kid) {
     Timing* t = c->tim;
@@ -126,6 +127,7 @@ static int ensure_storage(gp_ctx* c) {
     c->cfl_cached = false;
     c->spec = nullptr; c->padded = nullptr; c->kspec = nullptr; c->tabx = c->taby = c->tabz = nullptr;
     c->ztw = nullptr; c->src = nullptr; c->src_cached = false;
+    c->isofast = false; c->isoA = c->itwy = c->itwz = nullptr;
     if (g.poisson == GP_POISSON_PERIODIC) {
         c->spec = (cufftDoubleComplex*)take(((size_t)g.nx / 2 + 1) * g.ny * g.nz * sizeof(cufftDoubleComplex));
         c->tabx = (double*)take(((size_t)g.nx + g.ny + g.nz) * sizeof(double));
@@ -133,6 +135,15 @@ static int ensure_storage(gp_ctx* c) {
         c->tabz = c->taby + g.ny;
         c->ztw = (double*)take(2 * (size_t)g.nz * sizeof(double));
         if ((g.components & GP_GAS) && (g.components & GP_STARS)) c->src = (double*)take(N * sizeof(double));
+    } else if (g.poisson == GP_POISSON_ISOLATED && iso_pruned_supported(&g)) {
+        const size_t nxp = ((size_t)g.nx + 1 + 7) & ~(size_t)7, ny = g.ny, nz = g.nz;
+        c->isofast = true;
+        c->padded = (double*)take((nz + 2) * (ny + 2) * 2 * (size_t)g.nx * sizeof(double));
+        c->isoA = (double*)take((nz + 2) * (ny + 2) * nxp * 2 * sizeof(double));
+        c->spec = (cufftDoubleComplex*)take((nz + 2) * 2 * ny * nxp * sizeof(cufftDoubleComplex));
+        c->kspec = (double*)take(2 * nz * 2 * ny * nxp * sizeof(double));
+        c->itwy = (double*)take(2 * ny * 2 * sizeof(double));
+        c->itwz = (double*)take(2 * nz * 2 * sizeof(double));
     } else if (g.poisson == GP_POISSON_ISOLATED) {
         const size_t half = ((size_t)g.nx + 1) * (2 * (size_t)g.ny) * (2 * (size_t)g.nz);
         c->spec = (cufftDoubleComplex*)take(half * sizeof(cufftDoubleComplex));

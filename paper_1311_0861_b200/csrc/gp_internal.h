@@ -45,7 +45,7 @@ void set_error(const char* fmt, ...);
 
 // Kernels (and cuFFT executions) that can be timed one by one with CUDA events.
 enum KernelId { K_EUL_GAS = 0, K_LAG_GAS, K_EUL_BME, K_LAG_BME, K_CFL, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV,
-                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_NUM };
+                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_ISO_YFWD, K_ISO_ZFUSED, K_ISO_YINV, K_NUM };
 
 struct Timing {
     bool on = false;
@@ -88,6 +88,9 @@ struct gp_ctx {
     double* padded;                 // isolated: (2nx)(2ny)(2nz) real array
     double* kspec;                  // isolated: real spectrum of the 1/r kernel
     double* tabx; double* taby; double* tabz;   // periodic: 1 - (2/3) sin^2(pi k/N) per axis
+    bool isofast;                   // isolated: pruned transforms of isofft.cu (else full (2N)^3 cuFFT plans)
+    double* isoA;                   // isolated, pruned: x spectra of the data lines / of the kept lines
+    double* itwy; double* itwz;     // isolated, pruned: exp(-2 pi i k/2ny), exp(-2 pi i k/2nz)
     double* ztw;                    // periodic, fused z pass: exp(-2 pi i k/nz), nz complex values
     bool zfused;                    // periodic: 2-D batched cuFFT plans + the fused z pass (zpass.cu)
     double* src;                    // periodic, gas + stars: rho + n assembled here (by the fused step or k_source)
@@ -120,6 +123,12 @@ int poisson_setup(gp_ctx* c);
 void poisson_teardown(gp_ctx* c);
 int poisson_solve(gp_ctx* c);
 size_t poisson_storage_bytes(const gp_grid* g);
+
+// isofft.cu
+bool iso_pruned_supported(const gp_grid* g);
+size_t iso_pruned_storage_bytes(const gp_grid* g);
+int iso_pruned_setup(gp_ctx* c);
+int iso_pruned_solve(gp_ctx* c);
 
 // zpass.cu
 bool zpass_supported(int nz);

@@ -24,6 +24,7 @@ size_t poisson_storage_bytes(const gp_grid* g) {
         if ((g->components & GP_GAS) && (g->components & GP_STARS)) b += align256(nx * ny * nz * sizeof(double));   // rho + n
         return b;
     }
+    if (g->poisson == GP_POISSON_ISOLATED && iso_pruned_supported(g)) return iso_pruned_storage_bytes(g);
     if (g->poisson == GP_POISSON_ISOLATED) {
         const size_t half = (nx + 1) * (2 * ny) * (2 * nz);
         return align256(half * sizeof(cufftDoubleComplex)) + align256(half * sizeof(double)) +
@@ -161,6 +162,8 @@ int poisson_setup(gp_ctx* c) {
         for (int k = 0; k < nz; ++k) { const double s = std::sin(pi * k / nz); t[nx + ny + k] = 1.0 - 2.0 / 3.0 * s * s; }
         GP_CUDA(cudaMemcpyAsync(c->tabx, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
         GP_CUDA(cudaStreamSynchronize(c->stream));
+    } else if (c->g.poisson == GP_POISSON_ISOLATED && c->isofast) {
+        return iso_pruned_setup(c);
     } else if (c->g.poisson == GP_POISSON_ISOLATED) {
         GP_CUFFT(cufftPlan3d(&c->plan_fwd, 2 * nz, 2 * ny, 2 * nx, CUFFT_D2Z));
         GP_CUFFT(cufftPlan3d(&c->plan_inv, 2 * nz, 2 * ny, 2 * nx, CUFFT_Z2D));
@@ -232,6 +235,7 @@ int poisson_solve(gp_ctx* c) {
         GP_CUDA(cudaGetLastError());
         return launch_phi_ghost_bc(c, GP_BC_PERIODIC, GP_BC_PERIODIC, GP_BC_PERIODIC);
     }
+    if (c->isofast) return iso_pruned_solve(c);
     const size_t total = 8 * c->N, half = ((size_t)nx + 1) * (2 * (size_t)ny) * (2 * (size_t)nz);
     tic(c, K_PAD_SOURCE);
     k_pad_source<<<blocks_for(total), 256, 0, c->stream>>>(nx, ny, nz, rho, n, c->g.h * c->g.h * c->g.h, c->padded);

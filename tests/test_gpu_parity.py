@@ -65,12 +65,29 @@ def full_step(sim, ref, w, dt_cap=None):
     return dt
 
 
+REPORT = []          # (workload, grid, kind, field group, error) of every comparison, dumped at module teardown
+
+
+@pytest.fixture(scope="module", autouse=True)
+def parity_report():
+    yield
+    import json
+    import os
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    os.makedirs(out, exist_ok=True)
+    with open(os.path.join(out, "parity_report.json"), "w") as f:
+        json.dump(REPORT, f, indent=0)
+
+
 def check(sim, ref, w, tol, err):
+    kind = "max_1step" if err is err_max else "l1_nstep"
     for g in groups(w):
         e = err(sim, ref, g)
+        REPORT.append([w.name, [w.nx, w.ny, w.nz], kind, "+".join(g), float(e)])
         assert e <= tol, (w.name, g, e)
     if w.poisson != W.POISSON_NONE:
         e = err_max(sim, ref, ("phi",))
+        REPORT.append([w.name, [w.nx, w.ny, w.nz], kind, "phi", float(e)])
         assert e <= TOL_1STEP, (w.name, "phi", e)
 
 
@@ -300,3 +317,48 @@ def test_source_from_step_epilogue_equals_fresh_assembly(pkg, orc):
     a.solve_poisson()
     b.solve_poisson()
     assert np.array_equal(a.get("phi"), b.get("phi"))
+
+
+# ------------------------------------------------------------------------------------------------
+# isolated Poisson: pruned transforms (power-of-two ny, nz) and the full-cuFFT fallback, against
+# direct summation (the definition, PAPER.md:186 with the boundary reading G3) and the oracle
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims", [(4, 4, 4), (16, 8, 32), (8, 32, 4), (10, 16, 8), (6, 4, 64), (10, 12, 6), (8, 6, 8)])
+def test_isolated_poisson_against_direct_summation(pkg, orc, dims):
+    nx, ny, nz = dims
+    h, G = 0.1, 1.7
+    rng = np.random.default_rng(300 + nx + 7 * nz)
+    rho = rng.uniform(0.0, 1.0, (nz, ny, nx))
+    s = pkg.Simulation(nx, ny, nz, h, pkg.GP_GAS, pkg.GP_POISSON_ISOLATED, G=G, bc=(1, 1, 1))
+    s.set("rho", rho)
+    s.solve_poisson()
+    phi = s.get("phi")
+    ref = orc.poisson_direct(rho, h, G)
+    assert np.abs(phi - ref).max() <= 1e-11 * np.abs(ref).max()
+    s.set("rho", 2.0 * rho)                       # a second solve reuses plans, tables and work arrays
+    s.solve_poisson()
+    assert np.abs(s.get("phi") - 2.0 * ref).max() <= 2e-11 * np.abs(ref).max()
+
+
+def test_isolated_poisson_ghost_faces_drive_the_same_step_as_the_oracle(pkg, orc):
+    """The six ghost faces of Phi come from padded indices 2N-1 and N; a step of a cloud that touches
+    every face of a non-cubic box uses all of them."""
+    w = W.collapse(n=16, steps=1)
+    nx, ny, nz = 16, 8, 32
+    rng = np.random.default_rng(5)
+    st = {"rho": rng.uniform(0.5, 1.5, (nz, ny, nx))}
+    st["mx"] = 0.1 * st["rho"] * rng.uniform(-1, 1, (nz, ny, nx))
+    st["my"] = 0.1 * st["rho"] * rng.uniform(-1, 1, (nz, ny, nx))
+    st["mz"] = 0.1 * st["rho"] * rng.uniform(-1, 1, (nz, ny, nx))
+    st["E"] = 1.5 * st["rho"] + 0.5 * (st["mx"] ** 2 + st["my"] ** 2 + st["mz"] ** 2) / st["rho"]
+    sim = pkg.Simulation(nx, ny, nz, 0.05, pkg.GP_GAS, pkg.GP_POISSON_ISOLATED, G=1.0, gamma=w.gamma, bc=(1, 1, 1))
+    ref = orc.Oracle(nx, ny, nz, 0.05, orc.GAS, orc.POISSON_ISOLATED, 1.0, w.gamma, (1, 1, 1))
+    sim.set_state(st)
+    ref.set_state(st)
+    sim.solve_poisson()
+    ref.solve_poisson()
+    dt = ref.max_dt(0.2)
+    sim.step(dt)
+    ref.step(dt)
+    for g in GROUPS_GAS:
+        assert err_max(sim, ref, g) <= TOL_1STEP, g
