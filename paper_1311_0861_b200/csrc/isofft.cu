@@ -116,7 +116,7 @@ static int launch_col(gp_ctx* c, int n, int mode, const ColArgs& a, long long sl
         case 128: return launch_col_p<7, 8, 1>(c, mode, a, slabs, ncols, tw);
         case 256: return launch_col_p<8, 8, 1>(c, mode, a, slabs, ncols, tw);
         case 512: return launch_col_p<9, 4, 2>(c, mode, a, slabs, ncols, tw);
-        case 1024: return launch_col_p<10, 4, 1>(c, mode, a, slabs, ncols, tw);
+        case 1024: return launch_col_p<10, 4, 1>(c, mode, a, slabs, ncols, tw);   // <10, 2, 2> measured 30 % slower
     }
     set_error("isolated solve: transform length %d is not a supported power of two", n);
     return GP_ERR_UNSUPPORTED;
