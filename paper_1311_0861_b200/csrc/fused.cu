@@ -551,7 +551,8 @@ k_fused_gas(FusedArgs<NGAS> a) {
         const double phi_a = phi_load(pc, f.z0 - 2, zm, g.nz);
         double ir = frcp(rho);
         const double vz_a = mz * ir;
-        const double p_a = gm1 * (E - 0.5 * ((mx * mx + my * my) * ir + mz * vz_a));
+        // same expression as the main loop, so that a 1-D problem stays bitwise 1-D across the chunk edge
+        const double p_a = gm1 * (E - 0.5 * fma(mx, mx * ir, fma(my, my * ir, mz * vz_a)));
         const double rho_a = rho;
         zm = map_safe(f.z0 - 1, g.nz, g.bcz);
         off = f.base + (size_t)zm * f.nxny;
