@@ -1,0 +1,5 @@
+// Fused hydro step of the gas (fused_impl.cuh): footprint of 32 x 16 threads, 128 registers each.
+#define GP_FY 16
+#define GP_FUSED_NS fgas
+#define GP_FUSED_GAS 1
+#include "fused_impl.cuh"

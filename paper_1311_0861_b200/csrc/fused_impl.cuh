@@ -20,9 +20,17 @@
 #include "gp_internal.h"
 
 namespace gp {
+namespace GP_FUSED_NS {
 
-constexpr int FX = 32, FY = 16, PL = FX * FY;
+#ifndef GP_FY
+#define GP_FY 16
+#endif
+constexpr int FX = 32, FY = GP_FY, PL = FX * FY;
 constexpr int TXO = FX - 4, TYO = FY - 4;
+#define GP_KBOUNDS __launch_bounds__(PL, 1)
+#ifndef GP_BME_MERGE
+#define GP_BME_MERGE 0
+#endif
 
 // ---- fp64 reciprocal and reciprocal square root: MUFU seed + one cubically convergent step ----
 // seed relative error <= 2^-20  ->  after the step <= ~2^-59; final rounding ~1 ulp.
@@ -340,7 +348,7 @@ __device__ __forceinline__ void block_max_commit(double smax, int bad, unsigned 
         smax = threadIdx.x < FY ? scratch[threadIdx.x] : 0.0;
         bad = threadIdx.x < FY ? sbad[threadIdx.x] : 0;
 #pragma unroll
-        for (int o = 8; o > 0; o >>= 1) {
+        for (int o = 16; o > 0; o >>= 1) {
             smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
             bad |= __shfl_xor_sync(0xffffffffu, bad, o);
         }
@@ -351,6 +359,7 @@ __device__ __forceinline__ void block_max_commit(double smax, int bad, unsigned 
     }
 }
 
+#ifdef GP_FUSED_GAS
 // =================================================================================================
 // Gas: fields rho, mx, my, mz, E.
 // Shared planes (of PL doubles): (rho,p) pair 2, vx 1, vy 1, Phi 1, y-flux (P,PV) pair 2,
@@ -527,7 +536,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
     }
 }
 
-__global__ void __launch_bounds__(PL, 1)
+__global__ void GP_KBOUNDS
 k_fused_gas(FusedArgs<NGAS> a) {
     extern __shared__ double2 sm2[];
     double* sm = reinterpret_cast<double*>(sm2);
@@ -586,6 +595,9 @@ k_fused_gas(FusedArgs<NGAS> a) {
     block_max_commit(c.smax, c.bad, a.smax_bits, a.flag, S.rp);
 }
 
+#endif  // GP_FUSED_GAS
+
+#ifdef GP_FUSED_BME
 // =================================================================================================
 // Collisionless component: fields n, nu (3), nE_ij (6: xx xy xz yy yz zz).
 // Shared planes (of PL doubles): primitives (n,ux) (uy,uz) (Pxx,Pxz) (Pyy,Pyz) pairs 8 + Pxy 1 +
@@ -623,6 +635,31 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
     // B: x and y faces of plane j (hi face per thread)
     double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     double gx = 0.0, gy = 0.0;
+#if GP_BME_MERGE
+    {   // both solvers in ONE basic block so that their dependent chains interleave; rows 0 and FY-1
+        // (halo rows whose results are never used) run them on whatever they read
+        const int tn = t + FX, te = f.tx < FX - 1 ? t + 1 : t;
+        const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
+        const double2 x0 = lds2(S.nu + 2 * te), x1 = lds2(S.uu + 2 * te), x2 = lds2(S.px + 2 * te);
+        const double pxy_n = S.pxy[tn], pxy_e = S.pxy[te];
+        const double ury[3] = {y0.y, y1.x, y1.y}, urx[3] = {x0.y, x1.x, x1.y};
+        const double Ply[3] = {c.Pi[1], c.Pi[3], c.Pi[4]}, Plx[3] = {c.Pi[0], c.Pi[1], c.Pi[2]};
+        const double Pry[3] = {pxy_n, y2.x, y2.y}, Prx[3] = {x2.x, pxy_e, x2.y};
+        double Px[3], EFx[6];
+        bme_face<1>(c.n, c.u, Ply, y0.x, ury, Pry, Py, EFy);
+        bme_face<0>(c.n, c.u, Plx, x0.x, urx, Prx, Px, EFx);
+        double* fy = S.fy;
+        sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
+        sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
+        fy[4 * PP + t] = EFy[5];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) c.acc[q] -= th2 * (Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1));
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th4 * (EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1));
+        gx = (S.phi[t + 1] - S.phi[t - 1]) * inv2h;
+        gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
+    }
+#else
     if (f.ty <= FY - 2) {
         const int tn = t + FX;
         const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
@@ -650,6 +687,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
         gx = (S.phi[t + 1] - S.phi[t - 1]) * inv2h;
         gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
     }
+#endif
     __syncthreads();
 
     // C: y-flux difference, then everything of U*(j) but the upper z face
@@ -805,7 +843,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
     cp_async_commit();
 }
 
-__global__ void __launch_bounds__(PL, 1)
+__global__ void GP_KBOUNDS
 k_fused_bme(FusedArgs<NBME> a) {
     extern __shared__ double2 sm2[];
     double* sm = reinterpret_cast<double*>(sm2);
@@ -872,6 +910,8 @@ k_fused_bme(FusedArgs<NBME> a) {
     block_max_commit(c.smax, c.bad, a.smax_bits, a.flag, S.nu);
 }
 
+#endif  // GP_FUSED_BME
+
 // -------------------------------------------------------------------------------------------------
 // launches
 // -------------------------------------------------------------------------------------------------
@@ -919,21 +959,25 @@ static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, doub
     return GP_OK;
 }
 
-int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out) {
+#ifdef GP_FUSED_GAS
+static int launch_gas_impl(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out) {
     return launch_fused_t<NGAS>(c, k_fused_gas, 0, GAS_PLANES, K_FUSED_GAS, dt, d_dt, src_in, src_out);
 }
-
-int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt) {
+#endif
+#ifdef GP_FUSED_BME
+static int launch_bme_impl(gp_ctx* c, double dt, const double* d_dt) {
     return launch_fused_t<NBME>(c, k_fused_bme, NGAS, BME_PLANES, K_FUSED_BME, dt, d_dt);
 }
+#endif
 
+#ifdef GP_FUSED_GAS
 // evaluate the device reciprocal / reciprocal square root on n host-supplied values (self test)
 __global__ void k_math_selftest(int n, const double* __restrict__ x, double* __restrict__ rcp, double* __restrict__ rsq) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) { rcp[i] = frcp(x[i]); rsq[i] = frsqrt(x[i]); }
 }
 
-int math_selftest(int n, const double* x, double* rcp, double* rsq) {
+static int math_selftest_impl(int n, const double* x, double* rcp, double* rsq) {
     double *dx = nullptr;
     GP_CUDA(cudaMalloc(&dx, 3 * (size_t)n * sizeof(double)));
     cudaError_t e = cudaMemcpy(dx, x, (size_t)n * sizeof(double), cudaMemcpyHostToDevice);
@@ -946,5 +990,18 @@ int math_selftest(int n, const double* x, double* rcp, double* rsq) {
     GP_CUDA(e);
     return GP_OK;
 }
+#endif
+
+}  // namespace GP_FUSED_NS
+
+#ifdef GP_FUSED_GAS
+int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out) {
+    return GP_FUSED_NS::launch_gas_impl(c, dt, d_dt, src_in, src_out);
+}
+int math_selftest(int n, const double* x, double* rcp, double* rsq) { return GP_FUSED_NS::math_selftest_impl(n, x, rcp, rsq); }
+#endif
+#ifdef GP_FUSED_BME
+int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt) { return GP_FUSED_NS::launch_bme_impl(c, dt, d_dt); }
+#endif
 
 }  // namespace gp
