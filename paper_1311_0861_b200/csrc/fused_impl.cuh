@@ -301,9 +301,9 @@ struct Foot {
     int fix_src;
 };
 
-__device__ __forceinline__ Foot make_foot(const Geo& g, int zchunk, int row) {
+__device__ __forceinline__ Foot make_foot(const Geo& g, int zchunk) {
     Foot f;
-    f.tx = threadIdx.x; f.ty = row; f.t = f.ty * FX + f.tx;
+    f.tx = threadIdx.x; f.ty = threadIdx.y; f.t = f.ty * FX + f.tx;
     const int x0 = blockIdx.x * TXO, y0 = blockIdx.y * TYO;
     f.z0 = blockIdx.z * zchunk;
     f.z1 = min(g.nz, f.z0 + zchunk);
@@ -345,8 +345,8 @@ __device__ __forceinline__ void block_max_commit(double smax, int bad, unsigned 
     if (threadIdx.x == 0) { scratch[threadIdx.y] = smax; sbad[threadIdx.y] = bad; }
     __syncthreads();
     if (threadIdx.y == 0) {
-        smax = threadIdx.x < blockDim.y ? scratch[threadIdx.x] : 0.0;
-        bad = threadIdx.x < blockDim.y ? sbad[threadIdx.x] : 0;
+        smax = threadIdx.x < FY ? scratch[threadIdx.x] : 0.0;
+        bad = threadIdx.x < FY ? sbad[threadIdx.x] : 0;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
@@ -545,7 +545,7 @@ k_fused_gas(FusedArgs<NGAS> a) {
     S.ring = sm + 7 * PL; S.tz = S.ring + 3 * GAS_SLOT;
 
     const Geo& g = a.g;
-    const Foot f = make_foot(g, a.zchunk, threadIdx.y);
+    const Foot f = make_foot(g, a.zchunk);
     const int t = f.t;
     const double tau = a.dt_ptr ? *a.dt_ptr : a.dt_val;
     const double th = tau / a.h, inv2h = 0.5 / a.h, gm1 = a.gamma - 1.0;
@@ -619,14 +619,9 @@ struct BmeShared {
     double *nu, *uu, *px, *py, *pxy, *phi, *fy, *ring, *tz, *phst;
 };
 
-// what one cell carries from stage B to stage C across the first barrier
-struct BmeTmp { double Py[3], EFy[6], gx, gy; };
-
-// The iteration of plane j is cut at its barriers into stage functions so that a thread can run
-// them for RPT cells (footprint rows RPT*threadIdx.y .. +RPT-1) between the same two barriers.
 template <bool ST>
-__device__ __forceinline__ void bme_stage_B(const FusedArgs<NBME>& a, const Foot& f, const PhiCol& pc, const BmeShared& S,
-        BmeCarry& c, BmeTmp& T, int j, double tau, double th, double inv2h) {
+__device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f, const PhiCol& pc, const BmeShared& S,
+                                         BmeCarry& c, int j, double tau, double th, double inv2h) {
     const Geo& g = a.g;
     const int t = f.t;
     const double th2 = 0.5 * th, th4 = 0.25 * th;
@@ -638,14 +633,8 @@ __device__ __forceinline__ void bme_stage_B(const FusedArgs<NBME>& a, const Foot
     const bool stage_next = ST || j + 1 <= f.z1;
 
     // B: x and y faces of plane j (hi face per thread)
-    double (&Py)[3] = T.Py;
-    double (&EFy)[6] = T.EFy;
-    double &gx = T.gx, &gy = T.gy;
-#pragma unroll
-    for (int q = 0; q < 3; ++q) Py[q] = 0.0;
-#pragma unroll
-    for (int q = 0; q < 6; ++q) EFy[q] = 0.0;
-    gx = 0.0; gy = 0.0;
+    double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double gx = 0.0, gy = 0.0;
 #if GP_BME_MERGE
     {   // both solvers in ONE basic block so that their dependent chains interleave; rows 0 and FY-1
         // (halo rows whose results are never used) run them on whatever they read
@@ -699,24 +688,8 @@ __device__ __forceinline__ void bme_stage_B(const FusedArgs<NBME>& a, const Foot
         gy = (S.phi[t + FX] - S.phi[t - FX]) * inv2h;
     }
 #endif
-}
+    __syncthreads();
 
-template <bool ST>
-__device__ __forceinline__ void bme_stage_CE(const FusedArgs<NBME>& a, const Foot& f, const PhiCol& pc, const BmeShared& S,
-        BmeCarry& c, BmeTmp& T, int j, double tau, double th, double inv2h) {
-    const Geo& g = a.g;
-    const int t = f.t;
-    const double th2 = 0.5 * th, th4 = 0.25 * th;
-    const bool zout = g.bcz == GP_BC_OUTFLOW;
-    const bool top_copy = !ST && zout && j == g.nz;
-    const bool bot_dup = !ST && zout && j == 0;
-    const bool do_out = ST || j - 1 >= f.z0;
-    const bool do_wzp = ST || j >= f.z0;
-    const bool stage_next = ST || j + 1 <= f.z1;
-
-    const double (&Py)[3] = T.Py;
-    const double (&EFy)[6] = T.EFy;
-    const double gx = T.gx, gy = T.gy;
     // C: y-flux difference, then everything of U*(j) but the upper z face
     if (f.star_row) {
         const double* fy = S.fy + 2 * (t - FX);
@@ -802,15 +775,9 @@ __device__ __forceinline__ void bme_stage_CE(const FusedArgs<NBME>& a, const Foo
 #pragma unroll
     for (int q = 0; q < 6; ++q) c.Pi[q] = Pi_n[q];
     c.phim = c.phi0; c.phi0 = c.phin; c.phin = phi_n2;
-}
+    __syncthreads();
 
-template <bool ST>
-__device__ __forceinline__ void bme_stage_fix(const FusedArgs<NBME>& a, const Foot& f, const BmeShared& S, int j) {
-    const Geo& g = a.g;
-    const int t = f.t;
-    const bool bot_dup = !ST && g.bcz == GP_BC_OUTFLOW && j == 0;
-    double* rs = S.ring + ring_slot(j) * BME_SLOT;
-    {
+    if (f.block_fix) {
         if (f.fix) {
 #pragma unroll
             for (int P = 0; P < 5; ++P) {
@@ -821,24 +788,9 @@ __device__ __forceinline__ void bme_stage_fix(const FusedArgs<NBME>& a, const Fo
             const double2 v = lds2(S.tz + 2 * f.fix_src);
             sts2(S.tz + 2 * t, v.x, v.y);
         }
+        __syncthreads();
     }
 
-}
-
-template <bool ST>
-__device__ __forceinline__ void bme_stage_D(const FusedArgs<NBME>& a, const Foot& f, const PhiCol& pc, const BmeShared& S,
-        BmeCarry& c, BmeTmp& T, int j, double tau, double th, double inv2h) {
-    const Geo& g = a.g;
-    const int t = f.t;
-    const double th2 = 0.5 * th, th4 = 0.25 * th;
-    const bool zout = g.bcz == GP_BC_OUTFLOW;
-    const bool top_copy = !ST && zout && j == g.nz;
-    const bool bot_dup = !ST && zout && j == 0;
-    const bool do_out = ST || j - 1 >= f.z0;
-    const bool do_wzp = ST || j >= f.z0;
-    const bool stage_next = ST || j + 1 <= f.z1;
-
-    double* rs = S.ring + ring_slot(j) * BME_SLOT;
     // D: Lagrangian stage of plane j-1 (ring planes j-2, j-1, j)
     if (f.out_row) {
         const double Sz_new = sum9_wz(rs, t);             // 16 x
@@ -888,79 +840,10 @@ __device__ __forceinline__ void bme_stage_D(const FusedArgs<NBME>& a, const Foot
 #pragma unroll
         for (int q = 0; q < NBME; ++q) prefetch_l2(a.U[q] + off3);
     }
-}
-
-template <bool ST, int RPT>
-__device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot (&f)[RPT], const PhiCol (&pc)[RPT],
-                                         const BmeShared& S, BmeCarry (&c)[RPT], int j, double tau, double th, double inv2h) {
-    BmeTmp T[RPT];
-#pragma unroll
-    for (int r = 0; r < RPT; ++r) bme_stage_B<ST>(a, f[r], pc[r], S, c[r], T[r], j, tau, th, inv2h);
-    __syncthreads();
-#pragma unroll
-    for (int r = 0; r < RPT; ++r) bme_stage_CE<ST>(a, f[r], pc[r], S, c[r], T[r], j, tau, th, inv2h);
-    __syncthreads();
-    if (f[0].block_fix) {
-#pragma unroll
-        for (int r = 0; r < RPT; ++r) bme_stage_fix<ST>(a, f[r], S, j);
-        __syncthreads();
-    }
-#pragma unroll
-    for (int r = 0; r < RPT; ++r) bme_stage_D<ST>(a, f[r], pc[r], S, c[r], T[r], j, tau, th, inv2h);
     cp_async_commit();
 }
 
-#ifndef GP_BME_RPT
-#define GP_BME_RPT 1
-#endif
-constexpr int BME_RPT = GP_BME_RPT;      // footprint rows per thread
-
-// prologue of one cell: primitives of plane z0-2, then plane z0-1 with the z face between them
-__device__ __forceinline__ void bme_prologue(const FusedArgs<NBME>& a, const Foot& f, const PhiCol& pc, const BmeShared& S,
-                                             BmeCarry& c, double th) {
-    const Geo& g = a.g;
-    const int t = f.t;
-    c.Sz_prev = c.wzp_prev = c.smax = 0.0; c.bad = 0;
-    int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
-    size_t off = f.base + (size_t)zm * f.nxny;
-    double U0[NBME];
-#pragma unroll
-    for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
-    c.phim = phi_load(pc, f.z0 - 2, zm, g.nz);
-    const double n_a = U0[0];
-    double in = frcp(n_a);
-    const double u_a[3] = {U0[1] * in, U0[2] * in, U0[3] * in};
-    const double Pz_a[3] = {fma(-U0[1], u_a[2], U0[6]), fma(-U0[2], u_a[2], U0[8]), fma(-U0[3], u_a[2], U0[9])};
-    zm = map_safe(f.z0 - 1, g.nz, g.bcz);
-    off = f.base + (size_t)zm * f.nxny;
-#pragma unroll
-    for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
-    c.phi0 = phi_load(pc, f.z0 - 1, zm, g.nz);
-    c.n = U0[0]; c.in = frcp(c.n);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) c.u[d] = U0[1 + d] * c.in;
-    c.Pi[0] = fma(-U0[1], c.u[0], U0[4]); c.Pi[1] = fma(-U0[1], c.u[1], U0[5]); c.Pi[2] = fma(-U0[1], c.u[2], U0[6]);
-    c.Pi[3] = fma(-U0[2], c.u[1], U0[7]); c.Pi[4] = fma(-U0[2], c.u[2], U0[8]); c.Pi[5] = fma(-U0[3], c.u[2], U0[9]);
-    const double Pr[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
-    double Pz[3], EFz[6];
-    bme_face<2>(n_a, u_a, Pz_a, c.n, c.u, Pr, Pz, EFz);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) c.acc[d] = fma(0.5 * th, Pz[d], U0[1 + d]);
-#pragma unroll
-    for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(0.25 * th, EFz[q], U0[4 + q]);
-    sts2(S.nu + 2 * t, c.n, c.u[0]); sts2(S.uu + 2 * t, c.u[1], c.u[2]); sts2(S.px + 2 * t, c.Pi[0], c.Pi[2]);
-    sts2(S.py + 2 * t, c.Pi[3], c.Pi[4]); S.pxy[t] = c.Pi[1]; S.phi[t] = c.phi0;
-    // stage plane z0 where U*(z0-1) will be written
-    zm = map_safe(f.z0, g.nz, g.bcz);
-    off = f.base + (size_t)zm * f.nxny;
-    double* st = S.ring + ring_slot(f.z0 - 1) * BME_SLOT + 2 * t;
-#pragma unroll
-    for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
-    c.phin = phi_load(pc, f.z0, zm, g.nz);
-    cp_async8(S.phst + t, phi_ptr(pc, f.z0 + 1, map_safe(f.z0 + 1, g.nz, g.bcz), g.nz));
-}
-
-__global__ void __launch_bounds__(PL / BME_RPT, 1)
+__global__ void GP_KBOUNDS
 k_fused_bme(FusedArgs<NBME> a) {
     extern __shared__ double2 sm2[];
     double* sm = reinterpret_cast<double*>(sm2);
@@ -969,32 +852,64 @@ k_fused_bme(FusedArgs<NBME> a) {
     S.fy = sm + 10 * PL; S.ring = sm + 19 * PL; S.tz = S.ring + 3 * BME_SLOT; S.phst = S.tz + 2 * PL;
 
     const Geo& g = a.g;
+    const Foot f = make_foot(g, a.zchunk);
+    const int t = f.t;
     const double tau = a.dt_ptr ? *a.dt_ptr : a.dt_val;
     const double th = tau / a.h, inv2h = 0.5 / a.h;
-    Foot f[BME_RPT];
-    PhiCol pc[BME_RPT];
-    BmeCarry c[BME_RPT];
+    const PhiCol pc = phi_col(g, a.phi, f.xv, f.yv, f.xm, f.ym);
+
+    BmeCarry c;
+    c.Sz_prev = c.wzp_prev = c.smax = 0.0; c.bad = 0;
+    {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
+        int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
+        size_t off = f.base + (size_t)zm * f.nxny;
+        double U0[NBME];
 #pragma unroll
-    for (int r = 0; r < BME_RPT; ++r) {
-        f[r] = make_foot(g, a.zchunk, threadIdx.y * BME_RPT + r);
-        pc[r] = phi_col(g, a.phi, f[r].xv, f[r].yv, f[r].xm, f[r].ym);
-        bme_prologue(a, f[r], pc[r], S, c[r], th);
+        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
+        c.phim = phi_load(pc, f.z0 - 2, zm, g.nz);
+        const double n_a = U0[0];
+        double in = frcp(n_a);
+        const double u_a[3] = {U0[1] * in, U0[2] * in, U0[3] * in};
+        const double Pz_a[3] = {fma(-U0[1], u_a[2], U0[6]), fma(-U0[2], u_a[2], U0[8]), fma(-U0[3], u_a[2], U0[9])};
+        zm = map_safe(f.z0 - 1, g.nz, g.bcz);
+        off = f.base + (size_t)zm * f.nxny;
+#pragma unroll
+        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
+        c.phi0 = phi_load(pc, f.z0 - 1, zm, g.nz);
+        c.n = U0[0]; c.in = frcp(c.n);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c.u[d] = U0[1 + d] * c.in;
+        c.Pi[0] = fma(-U0[1], c.u[0], U0[4]); c.Pi[1] = fma(-U0[1], c.u[1], U0[5]); c.Pi[2] = fma(-U0[1], c.u[2], U0[6]);
+        c.Pi[3] = fma(-U0[2], c.u[1], U0[7]); c.Pi[4] = fma(-U0[2], c.u[2], U0[8]); c.Pi[5] = fma(-U0[3], c.u[2], U0[9]);
+        const double Pr[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
+        double Pz[3], EFz[6];
+        bme_face<2>(n_a, u_a, Pz_a, c.n, c.u, Pr, Pz, EFz);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c.acc[d] = fma(0.5 * th, Pz[d], U0[1 + d]);
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] = fma(0.25 * th, EFz[q], U0[4 + q]);
+        sts2(S.nu + 2 * t, c.n, c.u[0]); sts2(S.uu + 2 * t, c.u[1], c.u[2]); sts2(S.px + 2 * t, c.Pi[0], c.Pi[2]);
+        sts2(S.py + 2 * t, c.Pi[3], c.Pi[4]); S.pxy[t] = c.Pi[1]; S.phi[t] = c.phi0;
+        // stage plane z0 where U*(z0-1) will be written
+        zm = map_safe(f.z0, g.nz, g.bcz);
+        off = f.base + (size_t)zm * f.nxny;
+        double* st = S.ring + ring_slot(f.z0 - 1) * BME_SLOT + 2 * t;
+#pragma unroll
+        for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
+        c.phin = phi_load(pc, f.z0, zm, g.nz);
+        cp_async8(S.phst + t, phi_ptr(pc, f.z0 + 1, map_safe(f.z0 + 1, g.nz, g.bcz), g.nz));
+        cp_async_commit();
     }
-    cp_async_commit();
     __syncthreads();
 
-    const int z0 = f[0].z0, z1 = f[0].z1;
-    int j = z0 - 1;
-    for (; j <= z0 && j <= z1; ++j) bme_iter<false, BME_RPT>(a, f, pc, S, c, j, tau, th, inv2h);
-    for (; j <= z1 - 1; ++j) bme_iter<true, BME_RPT>(a, f, pc, S, c, j, tau, th, inv2h);
-    for (; j <= z1; ++j) bme_iter<false, BME_RPT>(a, f, pc, S, c, j, tau, th, inv2h);
+    int j = f.z0 - 1;
+    for (; j <= f.z0 && j <= f.z1; ++j) bme_iter<false>(a, f, pc, S, c, j, tau, th, inv2h);
+    for (; j <= f.z1 - 1; ++j) bme_iter<true>(a, f, pc, S, c, j, tau, th, inv2h);
+    for (; j <= f.z1; ++j) bme_iter<false>(a, f, pc, S, c, j, tau, th, inv2h);
     cp_async_wait_all();
-    double smax = c[0].smax;
-    int bad = c[0].bad;
-#pragma unroll
-    for (int r = 1; r < BME_RPT; ++r) { smax = fmax(smax, c[r].smax); bad |= c[r].bad; }
-    block_max_commit(smax, bad, a.smax_bits, a.flag, S.nu);
+    block_max_commit(c.smax, c.bad, a.smax_bits, a.flag, S.nu);
 }
+
 #endif  // GP_FUSED_BME
 
 // -------------------------------------------------------------------------------------------------
@@ -1019,7 +934,7 @@ static int pick_zchunk(const gp_ctx* c, int tiles_xy) {
 
 template <int NF, class K>
 static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, double dt, const double* d_dt,
-                          const double* src_in = nullptr, double* src_out = nullptr, int rpt = 1) {
+                          const double* src_in = nullptr, double* src_out = nullptr) {
     FusedArgs<NF> a;
     a.src_in = src_in; a.src_out = src_out;
     a.g = Geo{c->g.nx, c->g.ny, c->g.nz, c->bc.x, c->bc.y, c->bc.z};
@@ -1037,7 +952,7 @@ static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, doub
         attr_done[NF == NGAS ? 0 : 1] = true;
     }
     tic(c, kid);
-    kernel<<<dim3(tx, ty, tz), dim3(FX, FY / rpt, 1), smem, c->stream>>>(a);
+    kernel<<<dim3(tx, ty, tz), dim3(FX, FY, 1), smem, c->stream>>>(a);
     toc(c);
     c->n_own++;
     GP_CUDA(cudaGetLastError());
@@ -1051,7 +966,7 @@ static int launch_gas_impl(gp_ctx* c, double dt, const double* d_dt, const doubl
 #endif
 #ifdef GP_FUSED_BME
 static int launch_bme_impl(gp_ctx* c, double dt, const double* d_dt) {
-    return launch_fused_t<NBME>(c, k_fused_bme, NGAS, BME_PLANES, K_FUSED_BME, dt, d_dt, nullptr, nullptr, BME_RPT);
+    return launch_fused_t<NBME>(c, k_fused_bme, NGAS, BME_PLANES, K_FUSED_BME, dt, d_dt);
 }
 #endif
 
