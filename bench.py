@@ -35,10 +35,6 @@ W = 8  # bytes per fp64 word
 # Algorithmic bytes per cell of each own kernel: every array the stage
 # must read or write crosses HBM once (SURVEY.md 8(a) in->out column, 8(d) for the fused forms).
 ALGO_BYTES_PER_CELL = {
-    "eulerian_gas": (5 + 1 + 4) * W,        # a-2: reads 5 fields + Phi, writes 4 (rho* = rho)
-    "lagrangian_gas": (5 + 5) * W,          # a-3
-    "eulerian_bme": (10 + 1 + 9) * W,       # a-4
-    "lagrangian_bme": (10 + 10) * W,        # a-5
     "hydro_gas_fused": (5 + 1 + 5) * W,     # 8(d): R5 + RPhi + W5
     "hydro_bme_fused": (10 + 1 + 10) * W,   # 8(d): R10 + RPhi + W10
     "cfl": 15 * W,                          # a-6

@@ -31,6 +31,12 @@ constexpr int TXO = FX - 4, TYO = FY - 4;
 #ifndef GP_BME_MERGE
 #define GP_BME_MERGE 0
 #endif
+// x neighbours of the Lagrangian stage: 1 = 128-bit shared-memory loads of the cells t-1, t+1; 0 = warp
+// shuffles of the centre value (two SHFL plus register moves per double).  With the register budget
+// of the present footprints the loads are faster (21.99 against 22.43 ms per 512^3 step).
+#ifndef GP_X_LDS
+#define GP_X_LDS 1
+#endif
 
 // ---- fp64 reciprocal and reciprocal square root: MUFU seed + one cubically convergent step ----
 // seed relative error <= 2^-20  ->  after the step <= ~2^-59; final rounding ~1 ulp.
@@ -236,7 +242,11 @@ __device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, con
     // whole warps only: the x neighbours are fetched by shuffle
     const double2 a0 = lds2(r0 + 2 * t), aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
     const double2 azp = lds2(rp + 2 * t);
+#if GP_X_LDS
+    const double2 axm = lds2(r0 + 2 * (t - 1)), axp = lds2(r0 + 2 * (t + 1));
+#else
     const double2 axm = from_left(a0), axp = from_right(a0);
+#endif
     const double d0 = c.c0 * a0.x, dxm = c.xm * axm.x, dxp = c.xp * axp.x, dym = c.ym * aym.x, dyp = c.yp * ayp.x,
                  dzp = c.zp * azp.x;
     out[0] = ((out[0] + d0) + (dxm + dxp)) + ((dym + dyp) + dzp);
@@ -244,7 +254,11 @@ __device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, con
     {
         const double2 b0 = lds2(r0 + PP + 2 * t), bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
         const double2 bzp = lds2(rp + PP + 2 * t);
+#if GP_X_LDS
+        const double2 bxm = lds2(r0 + PP + 2 * (t - 1)), bxp = lds2(r0 + PP + 2 * (t + 1));
+#else
         const double2 bxm = from_left(b0), bxp = from_right(b0);
+#endif
         out[1] = fma(dzp, bzp.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, fma(d0, b0.x, out[1]))))));
         out[2] = fma(dzp, bzp.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, fma(d0, b0.y, out[2]))))));
     }
@@ -254,7 +268,11 @@ __device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, con
         if (2 * P + 1 < NO) {
             const double2 e0 = lds2(r0 + o + 2 * t), eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
             const double2 ezp = lds2(rp + o + 2 * t);
+#if GP_X_LDS
+            const double2 exm = lds2(r0 + o + 2 * (t - 1)), exp_ = lds2(r0 + o + 2 * (t + 1));
+#else
             const double2 exm = from_left(e0), exp_ = from_right(e0);
+#endif
             out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, fma(c.c0, e0.x, out[4 + 2 * P]))))));
             out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, fma(c.c0, e0.y, out[5 + 2 * P]))))));
         } else {
