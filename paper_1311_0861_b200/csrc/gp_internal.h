@@ -112,7 +112,7 @@ int launch_cfl_from_cache(gp_ctx* c, double cfl);
 int launch_cfl_reset_next(gp_ctx* c);
 int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz);
 
-// fused.cu
+// fused_gas.cu, fused_bme.cu (fused_impl.cuh)
 // src_out != nullptr: also write rho + n of the new state there (src_in = the new n, or nullptr)
 int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out);
 int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt);

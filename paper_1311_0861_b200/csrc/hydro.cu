@@ -1,5 +1,5 @@
 // Stand-alone CFL reduction (used when the state was set from outside; after a step the fused
-// kernels of fused.cu have already folded the max signal speed of the new state) and the Phi
+// kernels of fused_impl.cuh have already folded the max signal speed of the new state) and the Phi
 // ghost faces.  fp64 throughout.
 #include "gp_internal.h"
 
