@@ -73,7 +73,7 @@ int gp_get_state(gp_ctx* ctx, int field, double* dst, int dst_on_device);
  * Isolated mode: zero-padded (2N)^3 convolution with the -G/r kernel (Hockney & Eastwood); the
  * six ghost faces of Phi are taken from padded indices 2N-1 and N.  The first isolated solve of a
  * context also builds the kernel spectrum, for which it allocates (and frees before returning)
- * temporary device scratch of about 32 N bytes with cudaMalloc: GP_ERR_ALLOC if that fails.
+ * temporary device scratch of about 128 bytes per cell with cudaMalloc: GP_ERR_ALLOC if that fails.
  * Any even nx, ny, nz is accepted; power-of-two sizes (nz in [8, 1024] periodic; ny, nz <= 512
  * isolated) take the fused / pruned transforms, other sizes plain cuFFT 3-D plans.
  * With both components and the periodic mode the source rho + n is normally the one the last
