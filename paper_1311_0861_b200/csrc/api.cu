@@ -108,13 +108,19 @@ static int ensure_storage(gp_ctx* c) {
     char* p = c->base;
     auto take = [&](size_t bytes) { char* r = p; p += align256(bytes); return r; };
     const size_t N = c->N;
-    for (int f = 0; f < NHYD; ++f) {
-        c->U[f] = c->Us[f] = nullptr;
-        if (field_enabled(g, f)) {
+    for (int f = 0; f < NHYD; ++f) c->U[f] = c->Us[f] = nullptr;
+    if (g.components & GP_GAS)
+        for (int f = 0; f < NGAS; ++f) {
             c->U[f] = (double*)take(N * sizeof(double));
             c->Us[f] = (double*)take(N * sizeof(double));
         }
-    }
+    if (g.components & GP_STARS)
+        for (int P = 0; P < NBME / 2; ++P) {      // pairs of fields, one double2 per cell (gp_internal.h, BSTR)
+            double* u = (double*)take(2 * N * sizeof(double));
+            double* us = (double*)take(2 * N * sizeof(double));
+            c->U[NGAS + 2 * P] = u; c->U[NGAS + 2 * P + 1] = u + 1;
+            c->Us[NGAS + 2 * P] = us; c->Us[NGAS + 2 * P + 1] = us + 1;
+        }
     c->phi = (double*)take(N * sizeof(double));
     const size_t face[3] = {(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny};
     for (int s = 0; s < 6; ++s) c->phig[s] = (double*)take(face[s / 2] * sizeof(double));
@@ -134,7 +140,7 @@ static int ensure_storage(gp_ctx* c) {
         c->taby = c->tabx + g.nx;
         c->tabz = c->taby + g.ny;
         c->ztw = (double*)take(2 * (size_t)g.nz * sizeof(double));
-        if ((g.components & GP_GAS) && (g.components & GP_STARS)) c->src = (double*)take(N * sizeof(double));
+        if (g.components & GP_STARS) c->src = (double*)take(N * sizeof(double));   // rho + n, or n alone (paired in the state)
     } else if (g.poisson == GP_POISSON_ISOLATED && iso_pruned_supported(&g)) {
         const size_t nxp = ((size_t)g.nx + 1 + 7) & ~(size_t)7, ny = g.ny, nz = g.nz;
         c->isofast = true;
@@ -296,8 +302,21 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     double* dst = field == GP_PHI ? c->phi : c->U[field];
-    GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
-    if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));   // the host buffer may be reused on return
+    if (field != GP_PHI && field >= NGAS) {
+        // paired layout: a host array lands contiguously in the pair's step target (free between steps),
+        // then one kernel interleaves it; a device array is interleaved directly
+        const double* from = src;
+        if (!on_device) {
+            double* scratch = c->Us[NGAS + ((field - NGAS) & ~1)];
+            GP_CUDA(cudaMemcpyAsync(scratch, src, c->N * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+            GP_CUDA(cudaStreamSynchronize(c->stream));
+            from = scratch;
+        }
+        if ((rc = launch_strided_copy(c, dst, BSTR, from, 1, c->N)) != GP_OK) return rc;
+    } else {
+        GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+        if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));   // the host buffer may be reused on return
+    }
     if (field == GP_PHI) return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
     c->cfl_cached = false;
     c->src_cached = false;
@@ -310,6 +329,15 @@ int gp_get_state(gp_ctx* c, int field, double* dst, int on_device) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     const double* src = field == GP_PHI ? c->phi : c->U[field];
+    if (field != GP_PHI && field >= NGAS) {
+        double* scratch = c->Us[NGAS + ((field - NGAS) & ~1)];
+        if ((rc = launch_strided_copy(c, on_device ? dst : scratch, 1, src, BSTR, c->N)) != GP_OK) return rc;
+        if (!on_device) {
+            GP_CUDA(cudaMemcpyAsync(dst, scratch, c->N * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            GP_CUDA(cudaStreamSynchronize(c->stream));
+        }
+        return GP_OK;
+    }
     GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
     if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));
     return GP_OK;

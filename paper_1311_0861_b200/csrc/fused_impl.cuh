@@ -167,6 +167,11 @@ __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gmem) : "memory");
 }
+// 16-byte variant for the paired collisionless fields (gp_internal.h, BSTR); .cg: no L1 allocation
+__device__ __forceinline__ void cp_async16(double* smem, const double* gmem) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
 __device__ __forceinline__ void prefetch_l2(const double* gmem) { asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem)); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -517,7 +522,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
                 face_vel_xy(S.tz, t, wxm, wxp, wym, wyp);
                 lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, c.wzp_prev, wzp);
                 // density of the other component for the Poisson source: asked for early, used last
-                if (a.src_in && f.is_out) n_other = a.src_in[f.base + (size_t)(j - 1) * f.nxny];
+                if (a.src_in && f.is_out) n_other = a.src_in[BSTR * (f.base + (size_t)(j - 1) * f.nxny)];
                 lagrange_lower<1>(S.ring + ring_slot(j - 2) * GAS_SLOT, t, lc, out);
                 emit = true;
             }
@@ -825,7 +830,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
                 if (f.is_out) {
                     const size_t off = f.base + (size_t)(j - 1) * f.nxny;
 #pragma unroll
-                    for (int q = 0; q < NBME; ++q) a.Un[q][off] = out[q];
+                    for (int P = 0; P < NBME / 2; ++P)
+                        *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
                     // CFL of the new state (reading G4): |u_d| + sqrt(3 Pi_dd / n)
                     const double inn = frcp(out[0]);
                     const int dd[3] = {4, 7, 9};
@@ -851,12 +857,12 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, const Foot& f
         const size_t off = f.base + (size_t)zm * f.nxny;
         double* st = S.ring + ring_slot(j + 1) * BME_SLOT + 2 * t;
 #pragma unroll
-        for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
+        for (int P = 0; P < NBME / 2; ++P) cp_async16(st + P * PP, a.U[2 * P] + BSTR * off);     // one pair per copy
         cp_async8(S.phst + t, phi_ptr(pc, j + 3, map_safe(j + 3, g.nz, g.bcz), g.nz));
         // pull plane j+3 into L2 so that the next staging is an L2 hit
         const size_t off3 = f.base + (size_t)map_safe(j + 3, g.nz, g.bcz) * f.nxny;
 #pragma unroll
-        for (int q = 0; q < NBME; ++q) prefetch_l2(a.U[q] + off3);
+        for (int P = 0; P < NBME / 2; ++P) prefetch_l2(a.U[2 * P] + BSTR * off3);
     }
     cp_async_commit();
 }
@@ -883,7 +889,7 @@ k_fused_bme(FusedArgs<NBME> a) {
         size_t off = f.base + (size_t)zm * f.nxny;
         double U0[NBME];
 #pragma unroll
-        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
+        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][BSTR * off];
         c.phim = phi_load(pc, f.z0 - 2, zm, g.nz);
         const double n_a = U0[0];
         double in = frcp(n_a);
@@ -892,7 +898,7 @@ k_fused_bme(FusedArgs<NBME> a) {
         zm = map_safe(f.z0 - 1, g.nz, g.bcz);
         off = f.base + (size_t)zm * f.nxny;
 #pragma unroll
-        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][off];
+        for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][BSTR * off];
         c.phi0 = phi_load(pc, f.z0 - 1, zm, g.nz);
         c.n = U0[0]; c.in = frcp(c.n);
 #pragma unroll
@@ -913,7 +919,7 @@ k_fused_bme(FusedArgs<NBME> a) {
         off = f.base + (size_t)zm * f.nxny;
         double* st = S.ring + ring_slot(f.z0 - 1) * BME_SLOT + 2 * t;
 #pragma unroll
-        for (int q = 0; q < NBME; ++q) cp_async8(st + (q >> 1) * PP + (q & 1), a.U[q] + off);
+        for (int P = 0; P < NBME / 2; ++P) cp_async16(st + P * PP, a.U[2 * P] + BSTR * off);
         c.phin = phi_load(pc, f.z0, zm, g.nz);
         cp_async8(S.phst + t, phi_ptr(pc, f.z0 + 1, map_safe(f.z0 + 1, g.nz, g.bcz), g.nz));
         cp_async_commit();

@@ -15,6 +15,11 @@ namespace gp {
 constexpr int NGAS = 5;
 constexpr int NBME = 10;
 constexpr int NHYD = NGAS + NBME;
+// The ten collisionless fields live in HBM as five arrays of pairs (n,nu_x) (nu_y,nu_z) (nE_xx,nE_xy)
+// (nE_xz,nE_yy) (nE_yz,nE_zz), one double2 per cell, so that the fused kernel stages and stores
+// 16 bytes per access into its paired shared-memory layout; U[NGAS+q] points at member q&1 of pair
+// q>>1 and consecutive cells are BSTR doubles apart.  Gas fields and Phi are plain arrays (stride 1).
+constexpr int BSTR = 2;
 
 // Grid geometry handed to kernels by value.
 struct Geo {
@@ -111,6 +116,8 @@ int launch_cfl(gp_ctx* c, double cfl);
 int launch_cfl_from_cache(gp_ctx* c, double cfl);
 int launch_cfl_reset_next(gp_ctx* c);
 int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz);
+// dst[i * dstride] = src[i * sstride], i < n (field copies between the plain and the paired layout)
+int launch_strided_copy(gp_ctx* c, double* dst, int dstride, const double* src, int sstride, size_t n);
 
 // fused_gas.cu, fused_bme.cu (fused_impl.cuh)
 // src_out != nullptr: also write rho + n of the new state there (src_in = the new n, or nullptr)

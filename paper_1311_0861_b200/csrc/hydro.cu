@@ -51,13 +51,13 @@ k_cfl(size_t N, int has_gas, int has_stars, ConstFields<NGAS> Ug, ConstFields<NB
             }
         }
         if (has_stars) {
-            const double nn = Ub.p[0][c];
+            const double nn = Ub.p[0][BSTR * c];
             if (!(nn > 0.0)) bad = 1;
             const double in = 1.0 / nn;
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                const double u = Ub.p[1 + d][c] * in;
-                const double Pdd = Ub.p[4 + sym(d, d)][c] - nn * u * u;
+                const double u = Ub.p[1 + d][BSTR * c] * in;
+                const double Pdd = Ub.p[4 + sym(d, d)][BSTR * c] - nn * u * u;
                 if (!(Pdd > 0.0)) bad = 1;
                 const double s = fabs(u) + sqrt(3.0 * Pdd * in);
                 if (!(s <= 1.7976931348623157e308)) bad = 1;
@@ -124,6 +124,12 @@ __global__ void k_phi_ghost(Geo g, const double* __restrict__ phi, double* gx0, 
     }
 }
 
+__global__ void __launch_bounds__(256)
+k_strided_copy(size_t n, double* __restrict__ dst, int dstride, const double* __restrict__ src, int sstride) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        dst[i * dstride] = src[i * sstride];
+}
+
 // --------------------------------------------------------------------------------------------
 // launches
 // --------------------------------------------------------------------------------------------
@@ -165,6 +171,15 @@ int launch_cfl_from_cache(gp_ctx* c, double cfl) {
 int launch_cfl_reset_next(gp_ctx* c) {
     k_cfl_begin<<<1, 1, 0, c->stream>>>(c->d_smax_next, c->d_flag_next);
     c->n_own += 1;
+    GP_CUDA(cudaGetLastError());
+    return GP_OK;
+}
+
+int launch_strided_copy(gp_ctx* c, double* dst, int dstride, const double* src, int sstride, size_t n) {
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_strided_copy<<<(unsigned)blocks, 256, 0, c->stream>>>(n, dst, dstride, src, sstride);
+    c->n_own++;
     GP_CUDA(cudaGetLastError());
     return GP_OK;
 }

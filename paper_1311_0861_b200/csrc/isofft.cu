@@ -150,7 +150,7 @@ k_iso_pad_x(int nx, size_t lines, const double* __restrict__ rho, const double* 
         if (i < (size_t)nx) {
             const size_t c = line * nx + i;
             if (rho) v += rho[c];
-            if (n) v += n[c];
+            if (n) v += n[BSTR * c];
             v *= h3;
         }
         R[q] = v;

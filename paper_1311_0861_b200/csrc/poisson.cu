@@ -21,7 +21,7 @@ size_t poisson_storage_bytes(const gp_grid* g) {
     if (g->poisson == GP_POISSON_PERIODIC) {
         size_t b = align256((nx / 2 + 1) * ny * nz * sizeof(cufftDoubleComplex)) + 3 * align256((nx + ny + nz) * sizeof(double));
         b += align256(2 * nz * sizeof(double));                                   // twiddles of the fused z pass
-        if ((g->components & GP_GAS) && (g->components & GP_STARS)) b += align256(nx * ny * nz * sizeof(double));   // rho + n
+        if (g->components & GP_STARS) b += align256(nx * ny * nz * sizeof(double));   // rho + n (n is paired in the state)
         return b;
     }
     if (g->poisson == GP_POISSON_ISOLATED && iso_pruned_supported(g)) return iso_pruned_storage_bytes(g);
@@ -39,7 +39,7 @@ k_source(size_t N, const double* __restrict__ rho, const double* __restrict__ n,
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (size_t)gridDim.x * blockDim.x) {
         double v = 0.0;
         if (rho) v += rho[c];
-        if (n) v += n[c];
+        if (n) v += n[BSTR * c];
         s[c] = v;
     }
 }
@@ -74,7 +74,7 @@ k_pad_source(int nx, int ny, int nz, const double* __restrict__ rho, const doubl
         if (i < (size_t)nx && j < (size_t)ny && k < (size_t)nz) {
             const size_t c = i + (size_t)nx * (j + (size_t)ny * k);
             if (rho) v += rho[c];
-            if (n) v += n[c];
+            if (n) v += n[BSTR * c];
             v *= h3;
         }
         padded[q] = v;
@@ -207,8 +207,8 @@ int poisson_solve(gp_ctx* c) {
         const size_t half = ((size_t)nx / 2 + 1) * ny * nz;
         // source rho + n: one component -> its density is transformed in place of a
         // copy; both -> c->src, already written by the fused step unless the state was set since
-        const double* s = rho && n ? c->src : (rho ? rho : n);
-        if (rho && n && !c->src_cached) {
+        const double* s = n ? c->src : rho;
+        if (n && !c->src_cached) {
             tic(c, K_SOURCE);
             k_source<<<blocks_for(c->N), 256, 0, c->stream>>>(c->N, rho, n, c->src);
             toc(c);
