@@ -109,11 +109,16 @@ static int ensure_storage(gp_ctx* c) {
     auto take = [&](size_t bytes) { char* r = p; p += align256(bytes); return r; };
     const size_t N = c->N;
     for (int f = 0; f < NHYD; ++f) c->U[f] = c->Us[f] = nullptr;
-    if (g.components & GP_GAS)
-        for (int f = 0; f < NGAS; ++f) {
-            c->U[f] = (double*)take(N * sizeof(double));
-            c->Us[f] = (double*)take(N * sizeof(double));
+    if (g.components & GP_GAS) {
+        for (int P = 0; P < NGASP / 2; ++P) {     // (rho,m_x) (m_y,m_z): one double2 per cell (gp_internal.h, BSTR)
+            double* u = (double*)take(2 * N * sizeof(double));
+            double* us = (double*)take(2 * N * sizeof(double));
+            c->U[2 * P] = u; c->U[2 * P + 1] = u + 1;
+            c->Us[2 * P] = us; c->Us[2 * P + 1] = us + 1;
         }
+        c->U[GP_E] = (double*)take(N * sizeof(double));
+        c->Us[GP_E] = (double*)take(N * sizeof(double));
+    }
     if (g.components & GP_STARS)
         for (int P = 0; P < NBME / 2; ++P) {      // pairs of fields, one double2 per cell (gp_internal.h, BSTR)
             double* u = (double*)take(2 * N * sizeof(double));
@@ -140,7 +145,7 @@ static int ensure_storage(gp_ctx* c) {
         c->taby = c->tabx + g.nx;
         c->tabz = c->taby + g.ny;
         c->ztw = (double*)take(2 * (size_t)g.nz * sizeof(double));
-        if (g.components & GP_STARS) c->src = (double*)take(N * sizeof(double));   // rho + n, or n alone (paired in the state)
+        c->src = (double*)take(N * sizeof(double));   // rho + n (the densities are paired in the state)
     } else if (g.poisson == GP_POISSON_ISOLATED && iso_pruned_supported(&g)) {
         const size_t nxp = ((size_t)g.nx + 1 + 7) & ~(size_t)7, ny = g.ny, nz = g.nz;
         c->isofast = true;
@@ -302,12 +307,12 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     double* dst = field == GP_PHI ? c->phi : c->U[field];
-    if (field != GP_PHI && field >= NGAS) {
+    if (field != GP_PHI && field_paired(field)) {
         // paired layout: a host array lands contiguously in the pair's step target (free between steps),
         // then one kernel interleaves it; a device array is interleaved directly
         const double* from = src;
         if (!on_device) {
-            double* scratch = c->Us[NGAS + ((field - NGAS) & ~1)];
+            double* scratch = c->Us[pair_base(field)];
             GP_CUDA(cudaMemcpyAsync(scratch, src, c->N * sizeof(double), cudaMemcpyHostToDevice, c->stream));
             GP_CUDA(cudaStreamSynchronize(c->stream));
             from = scratch;
@@ -329,8 +334,8 @@ int gp_get_state(gp_ctx* c, int field, double* dst, int on_device) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     const double* src = field == GP_PHI ? c->phi : c->U[field];
-    if (field != GP_PHI && field >= NGAS) {
-        double* scratch = c->Us[NGAS + ((field - NGAS) & ~1)];
+    if (field != GP_PHI && field_paired(field)) {
+        double* scratch = c->Us[pair_base(field)];
         if ((rc = launch_strided_copy(c, on_device ? dst : scratch, 1, src, BSTR, c->N)) != GP_OK) return rc;
         if (!on_device) {
             GP_CUDA(cudaMemcpyAsync(dst, scratch, c->N * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -385,8 +390,9 @@ int gp_step(gp_ctx* c, double dt) {
         for (int f = NGAS; f < NHYD; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
     }
     if (c->g.components & GP_GAS) {
-        double* src_out = c->src;          // non-null only with both components and the periodic solve
-        if ((rc = launch_fused_gas(c, dt, d_dt, src_out ? c->U[GP_N] : nullptr, src_out)) != GP_OK) return rc;
+        double* src_out = c->src;          // non-null only with the periodic solve
+        const double* n_new = (c->g.components & GP_STARS) ? c->U[GP_N] : nullptr;
+        if ((rc = launch_fused_gas(c, dt, d_dt, src_out ? n_new : nullptr, src_out)) != GP_OK) return rc;
         for (int f = 0; f < NGAS; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
         c->src_cached = src_out != nullptr;
     }

@@ -534,8 +534,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
         const int zm = map_safe(j + 2, g.nz, g.bcz);
         const size_t off = f.base + (size_t)zm * f.nxny;
         double* st = S.ring + ring_slot(j + 1) * GAS_SLOT;
-        cp_async8(st + 2 * t, a.U[0] + off); cp_async8(st + 2 * t + 1, a.U[1] + off);
-        cp_async8(st + PP + 2 * t, a.U[2] + off); cp_async8(st + PP + 2 * t + 1, a.U[3] + off);
+        cp_async16(st + 2 * t, a.U[0] + BSTR * off); cp_async16(st + PP + 2 * t, a.U[2] + BSTR * off);   // pairs
         cp_async8(st + 2 * PP + 2 * t, a.U[4] + off);
         cp_async8(st + 2 * PP + 2 * t + 1, phi_ptr(pc, j + 2, zm, g.nz));
     }
@@ -545,7 +544,9 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, const Foot& f
         if (f.is_out) {
             const size_t off = f.base + (size_t)(j - 1) * f.nxny;
 #pragma unroll
-            for (int q = 0; q < NGAS; ++q) a.Un[q][off] = out[q];
+            for (int P = 0; P < NGASP / 2; ++P)
+                *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
+            a.Un[4][off] = out[4];
             if (a.src_out) a.src_out[off] = out[0] + n_other;
             // CFL of the new state (reading G4)
             const double irn = frcp(out[0]);
@@ -579,7 +580,7 @@ k_fused_gas(FusedArgs<NGAS> a) {
     {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
         int zm = map_safe(f.z0 - 2, g.nz, g.bcz);
         size_t off = f.base + (size_t)zm * f.nxny;
-        double rho = a.U[0][off], mx = a.U[1][off], my = a.U[2][off], mz = a.U[3][off], E = a.U[4][off];
+        double rho = a.U[0][BSTR * off], mx = a.U[1][BSTR * off], my = a.U[2][BSTR * off], mz = a.U[3][BSTR * off], E = a.U[4][off];
         const double phi_a = phi_load(pc, f.z0 - 2, zm, g.nz);
         double ir = frcp(rho);
         const double vz_a = mz * ir;
@@ -588,7 +589,7 @@ k_fused_gas(FusedArgs<NGAS> a) {
         const double rho_a = rho;
         zm = map_safe(f.z0 - 1, g.nz, g.bcz);
         off = f.base + (size_t)zm * f.nxny;
-        rho = a.U[0][off]; mx = a.U[1][off]; my = a.U[2][off]; mz = a.U[3][off]; E = a.U[4][off];
+        rho = a.U[0][BSTR * off]; mx = a.U[1][BSTR * off]; my = a.U[2][BSTR * off]; mz = a.U[3][BSTR * off]; E = a.U[4][off];
         const double phi_b = phi_load(pc, f.z0 - 1, zm, g.nz);
         ir = frcp(rho);
         c.rho = rho; c.ir = ir; c.vx = mx * ir; c.vy = my * ir; c.vz = mz * ir;
@@ -602,8 +603,7 @@ k_fused_gas(FusedArgs<NGAS> a) {
         zm = map_safe(f.z0, g.nz, g.bcz);
         off = f.base + (size_t)zm * f.nxny;
         double* st = S.ring + ring_slot(f.z0 - 1) * GAS_SLOT;
-        cp_async8(st + 2 * t, a.U[0] + off); cp_async8(st + 2 * t + 1, a.U[1] + off);
-        cp_async8(st + PP + 2 * t, a.U[2] + off); cp_async8(st + PP + 2 * t + 1, a.U[3] + off);
+        cp_async16(st + 2 * t, a.U[0] + BSTR * off); cp_async16(st + PP + 2 * t, a.U[2] + BSTR * off);   // pairs
         cp_async8(st + 2 * PP + 2 * t, a.U[4] + off);
         cp_async8(st + 2 * PP + 2 * t + 1, phi_ptr(pc, f.z0, zm, g.nz));
         cp_async_commit();

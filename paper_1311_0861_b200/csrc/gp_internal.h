@@ -15,11 +15,15 @@ namespace gp {
 constexpr int NGAS = 5;
 constexpr int NBME = 10;
 constexpr int NHYD = NGAS + NBME;
-// The ten collisionless fields live in HBM as five arrays of pairs (n,nu_x) (nu_y,nu_z) (nE_xx,nE_xy)
-// (nE_xz,nE_yy) (nE_yz,nE_zz), one double2 per cell, so that the fused kernel stages and stores
-// 16 bytes per access into its paired shared-memory layout; U[NGAS+q] points at member q&1 of pair
-// q>>1 and consecutive cells are BSTR doubles apart.  Gas fields and Phi are plain arrays (stride 1).
+// The state lives in HBM as arrays of field PAIRS, one double2 per cell: gas (rho,m_x) (m_y,m_z),
+// collisionless (n,nu_x) (nu_y,nu_z) (nE_xx,nE_xy) (nE_xz,nE_yy) (nE_yz,nE_zz), so that the fused
+// kernels stage and store 16 bytes per access straight into their paired shared-memory layout.
+// U[f] of a paired field points at its member of the pair and consecutive cells are BSTR doubles
+// apart.  The gas energy and Phi are plain arrays (stride 1).
 constexpr int BSTR = 2;
+constexpr int NGASP = 4;          // gas fields 0..3 are paired, field 4 (energy) is plain
+inline bool field_paired(int f) { return f < NGASP || (f >= NGAS && f < NHYD); }
+inline int pair_base(int f) { return f < NGAS ? (f & ~1) : NGAS + ((f - NGAS) & ~1); }
 
 // Grid geometry handed to kernels by value.
 struct Geo {

@@ -18,11 +18,11 @@ struct GasPrim { double rho, v[3], p; };
 
 __device__ __forceinline__ GasPrim gas_prim(const ConstFields<NGAS>& U, size_t c, double gm1) {
     GasPrim w;
-    w.rho = U.p[0][c];
+    w.rho = U.p[0][BSTR * c];
     const double ir = 1.0 / w.rho;
-    w.v[0] = U.p[1][c] * ir;
-    w.v[1] = U.p[2][c] * ir;
-    w.v[2] = U.p[3][c] * ir;
+    w.v[0] = U.p[1][BSTR * c] * ir;
+    w.v[1] = U.p[2][BSTR * c] * ir;
+    w.v[2] = U.p[3][BSTR * c] * ir;
     w.p = gm1 * (U.p[4][c] - 0.5 * w.rho * (w.v[0] * w.v[0] + w.v[1] * w.v[1] + w.v[2] * w.v[2]));
     return w;
 }

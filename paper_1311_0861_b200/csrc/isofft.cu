@@ -149,7 +149,7 @@ k_iso_pad_x(int nx, size_t lines, const double* __restrict__ rho, const double* 
         double v = 0.0;
         if (i < (size_t)nx) {
             const size_t c = line * nx + i;
-            if (rho) v += rho[c];
+            if (rho) v += rho[BSTR * c];
             if (n) v += n[BSTR * c];
             v *= h3;
         }

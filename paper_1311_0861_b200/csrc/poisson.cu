@@ -21,7 +21,7 @@ size_t poisson_storage_bytes(const gp_grid* g) {
     if (g->poisson == GP_POISSON_PERIODIC) {
         size_t b = align256((nx / 2 + 1) * ny * nz * sizeof(cufftDoubleComplex)) + 3 * align256((nx + ny + nz) * sizeof(double));
         b += align256(2 * nz * sizeof(double));                                   // twiddles of the fused z pass
-        if (g->components & GP_STARS) b += align256(nx * ny * nz * sizeof(double));   // rho + n (n is paired in the state)
+        b += align256(nx * ny * nz * sizeof(double));   // rho + n (the densities are paired in the state)
         return b;
     }
     if (g->poisson == GP_POISSON_ISOLATED && iso_pruned_supported(g)) return iso_pruned_storage_bytes(g);
@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(256)
 k_source(size_t N, const double* __restrict__ rho, const double* __restrict__ n, double* __restrict__ s) {
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (size_t)gridDim.x * blockDim.x) {
         double v = 0.0;
-        if (rho) v += rho[c];
+        if (rho) v += rho[BSTR * c];
         if (n) v += n[BSTR * c];
         s[c] = v;
     }
@@ -73,7 +73,7 @@ k_pad_source(int nx, int ny, int nz, const double* __restrict__ rho, const doubl
         double v = 0.0;
         if (i < (size_t)nx && j < (size_t)ny && k < (size_t)nz) {
             const size_t c = i + (size_t)nx * (j + (size_t)ny * k);
-            if (rho) v += rho[c];
+            if (rho) v += rho[BSTR * c];
             if (n) v += n[BSTR * c];
             v *= h3;
         }
@@ -205,10 +205,10 @@ int poisson_solve(gp_ctx* c) {
     const double pi = 3.14159265358979323846;
     if (c->g.poisson == GP_POISSON_PERIODIC) {
         const size_t half = ((size_t)nx / 2 + 1) * ny * nz;
-        // source rho + n: one component -> its density is transformed in place of a
-        // copy; both -> c->src, already written by the fused step unless the state was set since
-        const double* s = n ? c->src : rho;
-        if (n && !c->src_cached) {
+        // source rho + n in c->src (the densities are paired in the state, cuFFT wants a plain
+        // array): already written by the fused step unless the state was set since, or stars only
+        const double* s = c->src;
+        if (!c->src_cached) {
             tic(c, K_SOURCE);
             k_source<<<blocks_for(c->N), 256, 0, c->stream>>>(c->N, rho, n, c->src);
             toc(c);
