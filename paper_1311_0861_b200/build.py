@@ -21,7 +21,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC", "-o", LIB] + sources() + ["-lcufft"]
+           "-shared", "-Xcompiler", "-fPIC", "-o", LIB] + os.environ.get("GP_NVCC_FLAGS", "").split() + sources() + ["-lcufft"]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

@@ -20,7 +20,7 @@ void set_error(const char* fmt, ...) {
 static inline size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
 static const char* const kKernelNames[K_NUM] = {
-    "eulerian_gas", "lagrangian_gas", "eulerian_bme", "lagrangian_bme", "cfl", "poisson_source", "cufft_forward",
+    "cfl", "poisson_source", "cufft_forward",
     "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract",
     "hydro_gas_fused", "hydro_bme_fused", "poisson_zpass_green", "poisson_iso_yfwd", "poisson_iso_zfused",
     "poisson_iso_yinv"};
@@ -69,18 +69,14 @@ static bool field_enabled(const gp_grid& g, int f) {
     return f < NGAS ? (g.components & GP_GAS) != 0 : (g.components & GP_STARS) != 0;
 }
 
-static size_t ghost_elems(const gp_grid& g) {
-    return 2 * ((size_t)g.ny * g.nz + (size_t)g.nx * g.nz + (size_t)g.nx * g.ny);
-}
-
 static size_t storage_bytes(const gp_grid& g) {
     const size_t N = (size_t)g.nx * g.ny * g.nz;
     const size_t fb = align256(N * sizeof(double));
     size_t nf = 0;
     if (g.components & GP_GAS) nf += NGAS;
     if (g.components & GP_STARS) nf += NBME;
-    size_t b = (2 * nf + 1) * fb;                     // U, the step's target, Phi
-    b += 6 * align256(ghost_elems(g) / 2 * sizeof(double));   // generous: each face <= half of the total
+    size_t b = 2 * nf * fb;                           // U and the step's target
+    b += align256(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double));   // Phi with two ghost layers
     b += 256;                                         // dt, smax, flag
     b += poisson_storage_bytes(&g);
     return b;
@@ -126,9 +122,7 @@ static int ensure_storage(gp_ctx* c) {
             c->U[NGAS + 2 * P] = u; c->U[NGAS + 2 * P + 1] = u + 1;
             c->Us[NGAS + 2 * P] = us; c->Us[NGAS + 2 * P + 1] = us + 1;
         }
-    c->phi = (double*)take(N * sizeof(double));
-    const size_t face[3] = {(size_t)g.ny * g.nz, (size_t)g.nx * g.nz, (size_t)g.nx * g.ny};
-    for (int s = 0; s < 6; ++s) c->phig[s] = (double*)take(face[s / 2] * sizeof(double));
+    c->phip = (double*)take(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double));
     char* small = take(256);
     c->d_dt = (double*)small;
     c->d_smax = (unsigned long long*)(small + 64);
@@ -168,6 +162,22 @@ static int ensure_storage(gp_ctx* c) {
     // zero state, Phi and its ghost faces (GP_POISSON_NONE with Phi never set means no gravity)
     GP_CUDA(cudaMemsetAsync(c->base, 0, (size_t)(p - c->base), c->stream));
     c->ready = true;
+    return GP_OK;
+}
+
+// Copy Phi between a plain nx*ny*nz array (host or device) and the interior of the padded array.
+static int copy_phi(gp_ctx* c, double* plain, bool on_device, bool to_ctx) {
+    const gp_grid& g = c->g;
+    cudaMemcpy3DParms p = {};
+    const cudaPitchedPtr pad = make_cudaPitchedPtr(c->phip, (size_t)phi_pitch(g.nx) * sizeof(double), (size_t)phi_pitch(g.nx), (size_t)g.ny + 4);
+    const cudaPitchedPtr lin = make_cudaPitchedPtr(plain, (size_t)g.nx * sizeof(double), (size_t)g.nx, (size_t)g.ny);
+    const cudaPos in = make_cudaPos(2 * sizeof(double), 2, 2), zero = make_cudaPos(0, 0, 0);
+    p.srcPtr = to_ctx ? lin : pad; p.srcPos = to_ctx ? zero : in;
+    p.dstPtr = to_ctx ? pad : lin; p.dstPos = to_ctx ? in : zero;
+    p.extent = make_cudaExtent((size_t)g.nx * sizeof(double), (size_t)g.ny, (size_t)g.nz);
+    p.kind = on_device ? cudaMemcpyDeviceToDevice : (to_ctx ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost);
+    GP_CUDA(cudaMemcpy3DAsync(&p, c->stream));
+    if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));
     return GP_OK;
 }
 
@@ -306,8 +316,12 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     if (!field_enabled(c->g, field)) { set_error("gp_set_state: field %d is not enabled", field); return GP_ERR_ARG; }
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
-    double* dst = field == GP_PHI ? c->phi : c->U[field];
-    if (field != GP_PHI && field_paired(field)) {
+    if (field == GP_PHI) {
+        if ((rc = copy_phi(c, const_cast<double*>(src), on_device != 0, true)) != GP_OK) return rc;
+        return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
+    }
+    double* dst = c->U[field];
+    if (field_paired(field)) {
         // paired layout: a host array lands contiguously in the pair's step target (free between steps),
         // then one kernel interleaves it; a device array is interleaved directly
         const double* from = src;
@@ -322,7 +336,6 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
         GP_CUDA(cudaMemcpyAsync(dst, src, c->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
         if (!on_device) GP_CUDA(cudaStreamSynchronize(c->stream));   // the host buffer may be reused on return
     }
-    if (field == GP_PHI) return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
     c->cfl_cached = false;
     c->src_cached = false;
     return GP_OK;
@@ -333,8 +346,9 @@ int gp_get_state(gp_ctx* c, int field, double* dst, int on_device) {
     if (!field_enabled(c->g, field)) { set_error("gp_get_state: field %d is not enabled", field); return GP_ERR_ARG; }
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
-    const double* src = field == GP_PHI ? c->phi : c->U[field];
-    if (field != GP_PHI && field_paired(field)) {
+    if (field == GP_PHI) return copy_phi(c, dst, on_device != 0, false);
+    const double* src = c->U[field];
+    if (field_paired(field)) {
         double* scratch = c->Us[pair_base(field)];
         if ((rc = launch_strided_copy(c, on_device ? dst : scratch, 1, src, BSTR, c->N)) != GP_OK) return rc;
         if (!on_device) {

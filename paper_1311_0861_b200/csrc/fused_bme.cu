@@ -1,8 +1,12 @@
-// Fused hydro step of the collisionless component (fused_impl.cuh): footprint of 32 x 12 threads,
-// which leaves 168 registers per thread (no spills; measured 4 % faster than 32 x 16 at 128 with
-// spills) and room to run both face solvers of stage B in one basic block (another 1.5 %).
+// Fused hydro step of the collisionless component (fused_impl.cuh): footprint of 32 x 12 cells, twelve
+// Eulerian warps and four Lagrangian warps (512 threads, launched at 128 registers each and re-split with
+// setmaxnreg: the Eulerian warps carry 20 doubles of state per column and both face solvers of stage B in
+// one basic block).
 #define GP_FY 12
-#define GP_BME_MERGE 1
+#ifndef GP_REG_E
+#define GP_REG_E 136
+#define GP_REG_D 96
+#endif
 #define GP_FUSED_NS fbme
 #define GP_FUSED_BME 1
 #include "fused_impl.cuh"

@@ -41,20 +41,24 @@ struct ConstFields {
     const double* p[NF];
 };
 
-// Phi with its six ghost faces (x-, x+, y-, y+, z-, z+).  Face arrays are indexed
-// [j + ny*k], [i + nx*k], [i + nx*j].
-struct Phi {
-    const double* c;
-    const double* gx0; const double* gx1;
-    const double* gy0; const double* gy1;
-    const double* gz0; const double* gz1;
+// Phi lives in an array padded by TWO ghost layers per side: cell (i,j,k), i in [-2, nx+1] etc., sits at
+// p[(i+2) + pitch*((j+2) + py*(k+2))], pitch = nx+4 rounded up to even (rows stay 16-byte aligned), py = ny+4.
+// Layer 1 holds the ghost values of the Poisson mode (periodic solve: wrapped; isolated solve: the padded
+// convolution at indices -1 and n; user-set Phi: the hydro rule per axis); layer 2, edges and corners are
+// index maps of the same rule (wrap, or clamp for the isolated solve) and are only ever read for the U* of
+// periodic ghost cells.  The fused kernels therefore stage Phi rows without any case analysis.
+struct PhiPad {
+    const double* p;
+    int pitch, py;
 };
+inline int phi_pitch(int nx) { return (nx + 4 + 1) & ~1; }
+inline size_t phi_pad_elems(int nx, int ny, int nz) { return (size_t)phi_pitch(nx) * (ny + 4) * (nz + 4); }
 
 void set_error(const char* fmt, ...);
 
 // Kernels (and cuFFT executions) that can be timed one by one with CUDA events.
-enum KernelId { K_EUL_GAS = 0, K_LAG_GAS, K_EUL_BME, K_LAG_BME, K_CFL, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV,
-                K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT, K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_ISO_YFWD, K_ISO_ZFUSED, K_ISO_YINV, K_NUM };
+enum KernelId { K_CFL = 0, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV, K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT,
+                K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_ISO_YFWD, K_ISO_ZFUSED, K_ISO_YINV, K_NUM };
 
 struct Timing {
     bool on = false;
@@ -81,8 +85,7 @@ struct gp_ctx {
     bool ready;
     double* U[gp::NHYD];    // state U^n
     double* Us[gp::NHYD];   // target of the fused step (U^{n+1}); swapped with U after every step
-    double* phi;
-    double* phig[6];
+    double* phip;                   // Phi, padded by two ghost layers (PhiPad above)
     double* d_dt;                   // [0] = dt of the last gp_max_dt
     unsigned long long* d_smax;     // bit pattern of the running max signal speed
     int* d_flag;                    // != 0: bad state seen by the CFL reduction
@@ -119,7 +122,13 @@ void toc(gp_ctx* c);
 int launch_cfl(gp_ctx* c, double cfl);
 int launch_cfl_from_cache(gp_ctx* c, double cfl);
 int launch_cfl_reset_next(gp_ctx* c);
-int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz);
+// fill the ghost layers of Phi by wrap (GP_BC_PERIODIC) or clamp (GP_BC_OUTFLOW) per axis; keep_faces: leave the
+// six layer-1 faces as they are (the isolated solve has written them)
+int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz, bool keep_faces = false);
+inline PhiPad phipad_of(const gp_ctx* c) { return PhiPad{c->phip, phi_pitch(c->g.nx), c->g.ny + 4}; }
+inline double* phi_interior(const gp_ctx* c) {      // address of cell (0,0,0)
+    return c->phip + 2 + (size_t)phi_pitch(c->g.nx) * (2 + (size_t)(c->g.ny + 4) * 2);
+}
 // dst[i * dstride] = src[i * sstride], i < n (field copies between the plain and the paired layout)
 int launch_strided_copy(gp_ctx* c, double* dst, int dstride, const double* src, int sstride, size_t n);
 

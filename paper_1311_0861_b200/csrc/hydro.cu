@@ -1,6 +1,6 @@
 // Stand-alone CFL reduction (used when the state was set from outside; after a step the fused
-// kernels of fused_impl.cuh have already folded the max signal speed of the new state) and the Phi
-// ghost faces.  fp64 throughout.
+// kernels of fused_impl.cuh have already folded the max signal speed of the new state) and the ghost
+// layers of the padded Phi.  fp64 throughout.
 #include "gp_internal.h"
 
 namespace gp {
@@ -102,25 +102,42 @@ __global__ void k_cfl_finish(const unsigned long long* smax_bits, const int* fla
     *dt = cfl * h / s;
 }
 
-// Phi ghost faces by a boundary rule (wrap or copy of the nearest interior value).
-__global__ void k_phi_ghost(Geo g, const double* __restrict__ phi, double* gx0, double* gx1, double* gy0,
-                            double* gy1, double* gz0, double* gz1) {
-    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const size_t nyz = (size_t)g.ny * g.nz, nxz = (size_t)g.nx * g.nz, nxy = (size_t)g.nx * g.ny;
-    if (t < nyz) {
-        const int j = (int)(t % g.ny), k = (int)(t / g.ny);
-        gx0[t] = phi[cell(g, g.bcx == GP_BC_PERIODIC ? g.nx - 1 : 0, j, k)];
-        gx1[t] = phi[cell(g, g.bcx == GP_BC_PERIODIC ? 0 : g.nx - 1, j, k)];
-    }
-    if (t < nxz) {
-        const int i = (int)(t % g.nx), k = (int)(t / g.nx);
-        gy0[t] = phi[cell(g, i, g.bcy == GP_BC_PERIODIC ? g.ny - 1 : 0, k)];
-        gy1[t] = phi[cell(g, i, g.bcy == GP_BC_PERIODIC ? 0 : g.ny - 1, k)];
-    }
-    if (t < nxy) {
-        const int i = (int)(t % g.nx), j = (int)(t / g.nx);
-        gz0[t] = phi[cell(g, i, j, g.bcz == GP_BC_PERIODIC ? g.nz - 1 : 0)];
-        gz1[t] = phi[cell(g, i, j, g.bcz == GP_BC_PERIODIC ? 0 : g.nz - 1)];
+// Ghost layers of the padded Phi (gp_internal.h, PhiPad) by a boundary rule per axis: wrap (GP_BC_PERIODIC) or
+// copy of the nearest interior value (GP_BC_OUTFLOW).  Per-axis index maps equal filling x, then y over the
+// x-extended range, then z: edges and corners included.  keep_faces: positions with exactly one coordinate
+// outside by one (the six ghost faces) already hold their values (isolated solve) and are left alone.
+__device__ __forceinline__ int ghost_map(int i, int n, int bc) {
+    if (bc == GP_BC_PERIODIC) return i < 0 ? i + n : (i >= n ? i - n : i);
+    return i < 0 ? 0 : (i >= n ? n - 1 : i);
+}
+
+__global__ void __launch_bounds__(256)
+k_phi_ghost(Geo g, double* __restrict__ pad, int pitch, int keep_faces) {
+    const int px = g.nx + 4, py = g.ny + 4;
+    // enumerate the ghost cells only: four z slabs, then four y rows of every interior plane, then four x columns
+    const size_t nzs = (size_t)4 * px * py, nys = (size_t)4 * px * g.nz, nxs = (size_t)4 * g.ny * g.nz;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < nzs + nys + nxs; q += (size_t)gridDim.x * blockDim.x) {
+        int I, J, K;      // padded coordinates
+        if (q < nzs) {
+            I = (int)(q % px); J = (int)(q / px % py); const int s = (int)(q / ((size_t)px * py));
+            K = s < 2 ? s : g.nz + s;
+        } else if (q < nzs + nys) {
+            const size_t r = q - nzs;
+            I = (int)(r % px); const int s = (int)(r / px % 4); K = 2 + (int)(r / ((size_t)4 * px));
+            J = s < 2 ? s : g.ny + s;
+        } else {
+            const size_t r = q - nzs - nys;
+            const int s = (int)(r % 4); J = 2 + (int)(r / 4 % g.ny); K = 2 + (int)(r / ((size_t)4 * g.ny));
+            I = s < 2 ? s : g.nx + s;
+        }
+        const int i = I - 2, j = J - 2, k = K - 2;
+        if (keep_faces) {
+            const int ox = i < 0 ? -i : (i >= g.nx ? i - g.nx + 1 : 0), oy = j < 0 ? -j : (j >= g.ny ? j - g.ny + 1 : 0),
+                      oz = k < 0 ? -k : (k >= g.nz ? k - g.nz + 1 : 0);
+            if (ox + oy + oz == 1) continue;
+        }
+        const int im = ghost_map(i, g.nx, g.bcx), jm = ghost_map(j, g.ny, g.bcy), km = ghost_map(k, g.nz, g.bcz);
+        pad[(size_t)I + (size_t)pitch * (J + (size_t)py * K)] = pad[(size_t)(im + 2) + (size_t)pitch * ((jm + 2) + (size_t)py * (km + 2))];
     }
 }
 
@@ -135,10 +152,6 @@ k_strided_copy(size_t n, double* __restrict__ dst, int dstride, const double* __
 // --------------------------------------------------------------------------------------------
 static Geo geo_of(const gp_ctx* c) {
     return Geo{c->g.nx, c->g.ny, c->g.nz, c->bc.x, c->bc.y, c->bc.z};
-}
-
-static Phi phi_of(const gp_ctx* c) {
-    return Phi{c->phi, c->phig[0], c->phig[1], c->phig[2], c->phig[3], c->phig[4], c->phig[5]};
 }
 
 int launch_cfl(gp_ctx* c, double cfl) {
@@ -184,15 +197,14 @@ int launch_strided_copy(gp_ctx* c, double* dst, int dstride, const double* src, 
     return GP_OK;
 }
 
-int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz) {
+int launch_phi_ghost_bc(gp_ctx* c, int bcx, int bcy, int bcz, bool keep_faces) {
     Geo g = geo_of(c);
     g.bcx = bcx; g.bcy = bcy; g.bcz = bcz;
-    size_t m = (size_t)g.ny * g.nz;
-    if ((size_t)g.nx * g.nz > m) m = (size_t)g.nx * g.nz;
-    if ((size_t)g.nx * g.ny > m) m = (size_t)g.nx * g.ny;
+    const size_t m = (size_t)4 * (g.nx + 4) * (g.ny + 4) + (size_t)4 * (g.nx + 4) * g.nz + (size_t)4 * g.ny * g.nz;
+    size_t blocks = (m + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
     tic(c, K_PHI_GHOST);
-    k_phi_ghost<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(g, c->phi, c->phig[0], c->phig[1], c->phig[2],
-                                                                   c->phig[3], c->phig[4], c->phig[5]);
+    k_phi_ghost<<<(unsigned)blocks, 256, 0, c->stream>>>(g, c->phip, phi_pitch(g.nx), keep_faces ? 1 : 0);
     toc(c);
     c->n_own++;
     GP_CUDA(cudaGetLastError());

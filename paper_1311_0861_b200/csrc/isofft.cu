@@ -88,11 +88,8 @@ template <int P, int C, int MINB, bool FWD, bool INV, bool MUL>
 static int launch_col_k(gp_ctx* c, const ColArgs& a, long long slabs, const double2* tw) {
     const int threads = (1 << P) / 8 * C;
     const size_t smem = (size_t)(1 << P) * C * sizeof(double2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        GP_CUDA(cudaFuncSetAttribute(k_colfft<P, C, MINB, FWD, INV, MUL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    // the opt-in is per device and cheap: set it on every launch (a context may live on any device)
+    GP_CUDA(cudaFuncSetAttribute(k_colfft<P, C, MINB, FWD, INV, MUL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_colfft<P, C, MINB, FWD, INV, MUL><<<(unsigned)(slabs * a.tiles), threads, smem, c->stream>>>(a, tw);
     GP_CUDA(cudaGetLastError());
     return GP_OK;
@@ -159,18 +156,20 @@ k_iso_pad_x(int nx, size_t lines, const double* __restrict__ rho, const double* 
 
 // R[(nz+2)][(ny+2)][2nx] -> Phi and its six ghost faces; plane / row n holds padded index n, plane /
 // row n+1 holds padded index 2n-1 (where the cyclic convolution is still exact, G3)
+// phi points at cell (0,0,0) of the ghost-padded Phi array (row pitch `pitch`, py rows per plane); the
+// ghost faces are its cells -1 and n.
 __global__ void __launch_bounds__(256)
-k_iso_extract(int nx, int ny, int nz, const double* __restrict__ R, double* __restrict__ phi,
-              double* gx0, double* gx1, double* gy0, double* gy1, double* gz0, double* gz1) {
+k_iso_extract(int nx, int ny, int nz, const double* __restrict__ R, double* __restrict__ phi, int pitch, int py) {
     const size_t mx = 2 * (size_t)nx, rows = (size_t)ny + 2;
     const size_t N = (size_t)nx * ny * nz;
     auto P = [&](size_t i, size_t j, size_t k) { return R[i + mx * (j + rows * k)]; };
+    auto F = [&](long long i, long long j, long long k) -> double& { return phi[i + (long long)pitch * (j + (long long)py * k)]; };
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (size_t)gridDim.x * blockDim.x) {
         const size_t i = c % nx, r = c / nx, j = r % ny, k = r / ny;
-        phi[c] = P(i, j, k);
-        if (i == 0) { gx0[j + (size_t)ny * k] = P(2 * (size_t)nx - 1, j, k); gx1[j + (size_t)ny * k] = P(nx, j, k); }
-        if (j == 0) { gy0[i + (size_t)nx * k] = P(i, ny + 1, k); gy1[i + (size_t)nx * k] = P(i, ny, k); }
-        if (k == 0) { gz0[i + (size_t)nx * j] = P(i, j, nz + 1); gz1[i + (size_t)nx * j] = P(i, j, nz); }
+        F(i, j, k) = P(i, j, k);
+        if (i == 0) { F(-1, j, k) = P(2 * (size_t)nx - 1, j, k); F(nx, j, k) = P(nx, j, k); }
+        if (j == 0) { F(i, -1, k) = P(i, ny + 1, k); F(i, ny, k) = P(i, ny, k); }
+        if (k == 0) { F(i, j, -1) = P(i, j, nz + 1); F(i, j, nz) = P(i, j, nz); }
     }
 }
 
@@ -223,13 +222,21 @@ int iso_pruned_setup(gp_ctx* c) {
     GP_CUDA(cudaStreamSynchronize(c->stream));
 
     int n[1] = {2 * nx}, rembed[1] = {2 * nx}, cembed[1] = {nxp};
-    GP_CUFFT(cufftPlanMany(&c->plan_fwd, 1, n, rembed, 1, 2 * nx, cembed, 1, nxp, CUFFT_D2Z, nz * ny));
-    GP_CUFFT(cufftPlanMany(&c->plan_inv, 1, n, cembed, 1, nxp, rembed, 1, 2 * nx, CUFFT_Z2D, (nz + 2) * (ny + 2)));
-    GP_CUFFT(cufftSetStream(c->plan_fwd, c->stream));
-    GP_CUFFT(cufftSetStream(c->plan_inv, c->stream));
-    c->fft_ready = true;
     // the pad columns nx+1 .. nxp-1 of A are never written by cuFFT: keep them finite
     GP_CUDA(cudaMemsetAsync(c->isoA, 0, (size_t)(nz + 2) * (ny + 2) * nxp * sizeof(double2), c->stream));
+    GP_CUFFT(cufftPlanMany(&c->plan_fwd, 1, n, rembed, 1, 2 * nx, cembed, 1, nxp, CUFFT_D2Z, nz * ny));
+    if (cufftPlanMany(&c->plan_inv, 1, n, cembed, 1, nxp, rembed, 1, 2 * nx, CUFFT_Z2D, (nz + 2) * (ny + 2)) != CUFFT_SUCCESS) {
+        cufftDestroy(c->plan_fwd);
+        set_error("isolated solve: cufftPlanMany (inverse x lines) failed");
+        return GP_ERR_CUFFT;
+    }
+    // From here on every failure destroys both plans, and fft_ready is set only once the kernel spectrum
+    // exists: a retry after a failed set-up repeats it instead of convolving with a zero spectrum.
+    auto fail = [&](int code) { cufftDestroy(c->plan_fwd); cufftDestroy(c->plan_inv); return code; };
+    if (cufftSetStream(c->plan_fwd, c->stream) != CUFFT_SUCCESS || cufftSetStream(c->plan_inv, c->stream) != CUFFT_SUCCESS) {
+        set_error("isolated solve: cufftSetStream failed");
+        return fail(GP_ERR_CUFFT);
+    }
 
     // kernel spectrum, once, through the same forward pipeline (unpruned: the kernel fills the padded grid)
     const size_t full = 8 * c->N, spec = (size_t)(2 * nz) * rowsB;
@@ -240,7 +247,7 @@ int iso_pruned_setup(gp_ctx* c) {
     if (e != cudaSuccess) {
         cudaFree(Kfull);
         set_error("isolated solve: %zu bytes of set-up scratch: %s", full * sizeof(double) + spec * sizeof(double2), cudaGetErrorString(e));
-        return GP_ERR_ALLOC;
+        return fail(GP_ERR_ALLOC);
     }
     cufftHandle plan_k;
     int rc = GP_OK;
@@ -264,13 +271,14 @@ int iso_pruned_setup(gp_ctx* c) {
         if (rc == GP_OK) rc = launch_col(c, 2 * nz, COL_FWD, a, 1, rowsB, (const double2*)c->itwz);
         k_iso_take_real<<<grid_for(spec), 256, 0, c->stream>>>(spec, T, c->kspec);
         c->n_own += 4; c->n_fft += 1;
-        cudaStreamSynchronize(c->stream);
+        const cudaError_t es = cudaStreamSynchronize(c->stream);
+        if (rc == GP_OK && es != cudaSuccess) { set_error("isolated solve: building the kernel spectrum: %s", cudaGetErrorString(es)); rc = GP_ERR_CUDA; }
         cufftDestroy(plan_k);
     } while (0);
     cudaFree(Kfull);
     cudaFree(T);
-    if (rc != GP_OK) return rc;
-    GP_CUDA(cudaGetLastError());
+    if (rc != GP_OK) return fail(rc);
+    c->fft_ready = true;
     return GP_OK;
 }
 
@@ -314,12 +322,12 @@ int iso_pruned_solve(gp_ctx* c) {
     GP_CUFFT(cufftExecZ2D(c->plan_inv, (cufftDoubleComplex*)A, c->padded));
     toc(c);
     tic(c, K_EXTRACT);
-    k_iso_extract<<<grid_for(c->N), 256, 0, c->stream>>>(nx, ny, nz, c->padded, c->phi, c->phig[0], c->phig[1], c->phig[2],
-                                                         c->phig[3], c->phig[4], c->phig[5]);
+    k_iso_extract<<<grid_for(c->N), 256, 0, c->stream>>>(nx, ny, nz, c->padded, phi_interior(c), phi_pitch(nx), ny + 4);
     toc(c);
     c->n_own += 5; c->n_fft += 2;
     GP_CUDA(cudaGetLastError());
-    return GP_OK;
+    // layer 2, edges and corners: never used by a result (outflow hydro boundaries), kept finite
+    return launch_phi_ghost_bc(c, GP_BC_OUTFLOW, GP_BC_OUTFLOW, GP_BC_OUTFLOW, true);
 }
 
 }  // namespace gp

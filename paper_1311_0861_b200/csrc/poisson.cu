@@ -6,7 +6,9 @@
 // Isolated mode: cyclic convolution on the zero-padded (2N)^3 grid with K(r) = 1/|r|,
 // K(0) = (3 ln((sqrt3+1)/(sqrt3-1)) - pi/2)/h (potential at the centre of a uniform cube);
 // Phi = -G * sum_j m_j K.  The six ghost faces of Phi are read from padded indices 2N-1 and N,
-// where the convolution is still exact.
+// where the convolution is still exact.  Phi is written straight into the interior of its ghost-padded
+// array (gp_internal.h, PhiPad): cuFFT's inverse transforms through an output embedding, the isolated
+// solves by their extraction kernels; k_phi_ghost then fills the ghost layers.
 #include <cmath>
 #include <vector>
 
@@ -111,19 +113,20 @@ k_mul_real(size_t total, const double* __restrict__ ks, double scale, cufftDoubl
     }
 }
 
-// Interior of the padded result -> Phi; padded indices 2N-1 and N -> the six ghost faces.
+// Interior of the (2N)^3 result -> Phi; its indices 2N-1 and N -> the six ghost faces (cells -1 and n).
+// phi points at cell (0,0,0) of the ghost-padded Phi array (row pitch `pitch`, py rows per plane).
 __global__ void __launch_bounds__(256)
-k_extract(int nx, int ny, int nz, const double* __restrict__ padded, double* __restrict__ phi,
-          double* gx0, double* gx1, double* gy0, double* gy1, double* gz0, double* gz1) {
+k_extract(int nx, int ny, int nz, const double* __restrict__ padded, double* __restrict__ phi, int pitch, int py) {
     const size_t mx = 2 * (size_t)nx, my = 2 * (size_t)ny;
     const size_t N = (size_t)nx * ny * nz;
     auto P = [&](size_t i, size_t j, size_t k) { return padded[i + mx * (j + my * k)]; };
+    auto F = [&](long long i, long long j, long long k) -> double& { return phi[i + (long long)pitch * (j + (long long)py * k)]; };
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (size_t)gridDim.x * blockDim.x) {
         const size_t i = c % nx, r = c / nx, j = r % ny, k = r / ny;
-        phi[c] = P(i, j, k);
-        if (i == 0) { gx0[j + (size_t)ny * k] = P(2 * (size_t)nx - 1, j, k); gx1[j + (size_t)ny * k] = P(nx, j, k); }
-        if (j == 0) { gy0[i + (size_t)nx * k] = P(i, 2 * (size_t)ny - 1, k); gy1[i + (size_t)nx * k] = P(i, ny, k); }
-        if (k == 0) { gz0[i + (size_t)nx * j] = P(i, j, 2 * (size_t)nz - 1); gz1[i + (size_t)nx * j] = P(i, j, nz); }
+        F(i, j, k) = P(i, j, k);
+        if (i == 0) { F(-1, j, k) = P(2 * (size_t)nx - 1, j, k); F(nx, j, k) = P(nx, j, k); }
+        if (j == 0) { F(i, -1, k) = P(i, 2 * (size_t)ny - 1, k); F(i, ny, k) = P(i, ny, k); }
+        if (k == 0) { F(i, j, -1) = P(i, j, 2 * (size_t)nz - 1); F(i, j, nz) = P(i, j, nz); }
     }
 }
 
@@ -136,13 +139,18 @@ static unsigned blocks_for(size_t n) {
 int poisson_setup(gp_ctx* c) {
     if (c->fft_ready) return GP_OK;
     const int nx = c->g.nx, ny = c->g.ny, nz = c->g.nz;
+    const int pitch = phi_pitch(nx), py = ny + 4;      // the inverse transform writes into the padded Phi
     if (c->g.poisson == GP_POISSON_PERIODIC) {
         c->zfused = zpass_supported(nz);
         if (c->zfused) {
             // batched 2-D real transforms over the xy planes; the z direction is zpass.cu's
-            int n[2] = {ny, nx}, rembed[2] = {ny, nx}, cembed[2] = {ny, nx / 2 + 1};
+            int n[2] = {ny, nx}, rembed[2] = {ny, nx}, cembed[2] = {ny, nx / 2 + 1}, pembed[2] = {py, pitch};
             GP_CUFFT(cufftPlanMany(&c->plan_fwd, 2, n, rembed, 1, ny * nx, cembed, 1, ny * (nx / 2 + 1), CUFFT_D2Z, nz));
-            GP_CUFFT(cufftPlanMany(&c->plan_inv, 2, n, cembed, 1, ny * (nx / 2 + 1), rembed, 1, ny * nx, CUFFT_Z2D, nz));
+            if (cufftPlanMany(&c->plan_inv, 2, n, cembed, 1, ny * (nx / 2 + 1), pembed, 1, py * pitch, CUFFT_Z2D, nz) != CUFFT_SUCCESS) {
+                cufftDestroy(c->plan_fwd);
+                set_error("gp_solve_poisson: cufftPlanMany (inverse, padded output) failed");
+                return GP_ERR_CUFFT;
+            }
             std::vector<double> w(2 * (size_t)nz);
             for (int k = 0; k < nz; ++k) {
                 const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)nz;
@@ -152,8 +160,13 @@ int poisson_setup(gp_ctx* c) {
             GP_CUDA(cudaMemcpyAsync(c->ztw, w.data(), w.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
             GP_CUDA(cudaStreamSynchronize(c->stream));
         } else {
+            int n[3] = {nz, ny, nx}, cembed[3] = {nz, ny, nx / 2 + 1}, pembed[3] = {nz + 4, py, pitch};
             GP_CUFFT(cufftPlan3d(&c->plan_fwd, nz, ny, nx, CUFFT_D2Z));
-            GP_CUFFT(cufftPlan3d(&c->plan_inv, nz, ny, nx, CUFFT_Z2D));
+            if (cufftPlanMany(&c->plan_inv, 3, n, cembed, 1, nz * ny * (nx / 2 + 1), pembed, 1, (nz + 4) * py * pitch, CUFFT_Z2D, 1) != CUFFT_SUCCESS) {
+                cufftDestroy(c->plan_fwd);
+                set_error("gp_solve_poisson: cufftPlanMany (inverse 3-D, padded output) failed");
+                return GP_ERR_CUFFT;
+            }
         }
         const double pi = 3.14159265358979323846;
         std::vector<double> t((size_t)nx + ny + nz);
@@ -166,25 +179,46 @@ int poisson_setup(gp_ctx* c) {
         return iso_pruned_setup(c);
     } else if (c->g.poisson == GP_POISSON_ISOLATED) {
         GP_CUFFT(cufftPlan3d(&c->plan_fwd, 2 * nz, 2 * ny, 2 * nx, CUFFT_D2Z));
-        GP_CUFFT(cufftPlan3d(&c->plan_inv, 2 * nz, 2 * ny, 2 * nx, CUFFT_Z2D));
+        if (cufftPlan3d(&c->plan_inv, 2 * nz, 2 * ny, 2 * nx, CUFFT_Z2D) != CUFFT_SUCCESS) {
+            cufftDestroy(c->plan_fwd);
+            set_error("gp_solve_poisson: cufftPlan3d (inverse) failed");
+            return GP_ERR_CUFFT;
+        }
     } else {
         set_error("gp_solve_poisson: context was created with GP_POISSON_NONE");
         return GP_ERR_UNSUPPORTED;
     }
-    GP_CUFFT(cufftSetStream(c->plan_fwd, c->stream));
-    GP_CUFFT(cufftSetStream(c->plan_inv, c->stream));
-    c->fft_ready = true;
-    if (c->g.poisson == GP_POISSON_ISOLATED) {
+    // From here on a failure must not leave half-built plans behind, and fft_ready is set only once the
+    // kernel spectrum exists: a retry after a failed set-up repeats it instead of convolving with zeros.
+    int rc = GP_OK;
+    if (cufftSetStream(c->plan_fwd, c->stream) != CUFFT_SUCCESS || cufftSetStream(c->plan_inv, c->stream) != CUFFT_SUCCESS) {
+        set_error("gp_solve_poisson: cufftSetStream failed");
+        rc = GP_ERR_CUFFT;
+    }
+    if (rc == GP_OK && c->g.poisson == GP_POISSON_ISOLATED) {
         // spectrum of the kernel, once: real because the kernel is even in every axis
         const size_t total = 8 * c->N, half = ((size_t)nx + 1) * (2 * (size_t)ny) * (2 * (size_t)nz);
         const double s3 = std::sqrt(3.0), pi = 3.14159265358979323846;
         const double kself = 3.0 * std::log((s3 + 1.0) / (s3 - 1.0)) - pi / 2.0;
         k_kernel_fill<<<blocks_for(total), 256, 0, c->stream>>>(nx, ny, nz, c->g.h, kself, c->padded);
-        GP_CUFFT(cufftExecD2Z(c->plan_fwd, c->padded, c->spec));
+        if (cufftExecD2Z(c->plan_fwd, c->padded, c->spec) != CUFFT_SUCCESS) {
+            set_error("gp_solve_poisson: kernel-spectrum transform failed");
+            rc = GP_ERR_CUFFT;
+        }
         k_take_real<<<blocks_for(half), 256, 0, c->stream>>>(half, c->spec, c->kspec);
         c->n_own += 2; c->n_fft += 1;
-        GP_CUDA(cudaGetLastError());
+        const cudaError_t e = cudaStreamSynchronize(c->stream);
+        if (rc == GP_OK && e != cudaSuccess) {
+            set_error("gp_solve_poisson: building the kernel spectrum: %s", cudaGetErrorString(e));
+            rc = GP_ERR_CUDA;
+        }
     }
+    if (rc != GP_OK) {
+        cufftDestroy(c->plan_fwd);
+        cufftDestroy(c->plan_inv);
+        return rc;
+    }
+    c->fft_ready = true;
     return GP_OK;
 }
 
@@ -229,7 +263,7 @@ int poisson_solve(gp_ctx* c) {
             toc(c);
         }
         tic(c, K_FFT_INV);
-        GP_CUFFT(cufftExecZ2D(c->plan_inv, c->spec, c->phi));
+        GP_CUFFT(cufftExecZ2D(c->plan_inv, c->spec, phi_interior(c)));
         toc(c);
         c->n_own += 1; c->n_fft += 2;
         GP_CUDA(cudaGetLastError());
@@ -250,12 +284,12 @@ int poisson_solve(gp_ctx* c) {
     GP_CUFFT(cufftExecZ2D(c->plan_inv, c->spec, c->padded));
     toc(c);
     tic(c, K_EXTRACT);
-    k_extract<<<blocks_for(c->N), 256, 0, c->stream>>>(nx, ny, nz, c->padded, c->phi, c->phig[0], c->phig[1], c->phig[2],
-                                                       c->phig[3], c->phig[4], c->phig[5]);
+    k_extract<<<blocks_for(c->N), 256, 0, c->stream>>>(nx, ny, nz, c->padded, phi_interior(c), phi_pitch(nx), ny + 4);
     toc(c);
     c->n_own += 3; c->n_fft += 2;
     GP_CUDA(cudaGetLastError());
-    return GP_OK;
+    // layer 2, edges and corners: never used by a result (outflow hydro boundaries), kept finite
+    return launch_phi_ghost_bc(c, GP_BC_OUTFLOW, GP_BC_OUTFLOW, GP_BC_OUTFLOW, true);
 }
 
 }  // namespace gp

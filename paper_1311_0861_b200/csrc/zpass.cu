@@ -81,11 +81,8 @@ static int launch_zpass_t(gp_ctx* c, double coef6) {
     const size_t plane = ((size_t)c->g.nx / 2 + 1) * c->g.ny;
     const int threads = (1 << P) / 8 * ZC;
     const size_t smem = (size_t)(1 << P) * ZC * sizeof(double2);
-    static bool attr_done = false;
-    if (!attr_done) {
-        GP_CUDA(cudaFuncSetAttribute(k_zpass_green<P, ZC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    // the opt-in is per device and cheap: set it on every launch (a context may live on any device)
+    GP_CUDA(cudaFuncSetAttribute(k_zpass_green<P, ZC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_zpass_green<P, ZC, MINB><<<(unsigned)((plane + ZC - 1) / ZC), threads, smem, c->stream>>>(
         plane, c->g.nx / 2 + 1, c->tabx, c->taby, c->tabz, (const double2*)c->ztw, coef6, (double2*)c->spec);
     GP_CUDA(cudaGetLastError());

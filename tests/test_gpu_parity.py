@@ -161,6 +161,29 @@ def test_minimum_grid_and_boundary_mixes(pkg, orc, bc):
     run_parity(pkg, orc, w, 5)
 
 
+@pytest.mark.parametrize("bc", [(1, 0, 1), (0, 1, 0), (1, 1, 0), (1, 1, 1)])
+def test_mixed_hydro_boundaries_under_the_periodic_solve(pkg, orc, bc):
+    """Periodic Poisson solve (Phi and its ghosts wrap on every axis) with outflow hydro boundaries on some
+    axes: the U* of a periodic ghost cell next to an outflow face takes grad Phi from the wrapped Phi."""
+    w = W.two_disks(n=32, rd_cells=3.2, zd_cells=1.28)
+    w.bc = bc
+    run_parity(pkg, orc, w, 6)
+
+
+def test_user_set_phi_with_mixed_boundaries(pkg, orc):
+    """GP_POISSON_NONE with a Phi handed in by the caller: its ghosts follow the hydro rule per axis."""
+    w = W.smooth_gas(dims=(36, 10, 12), kmax=2, amp=0.2, components=W.GAS | W.STARS)
+    w.bc = (1, 0, 1)
+    rng = np.random.default_rng(77)
+    phi = 0.3 * rng.standard_normal((w.nz, w.ny, w.nx))
+    sim, ref = make_pair(pkg, orc, w)
+    sim.set("phi", phi)
+    ref.set("phi", phi)
+    for _ in range(4):
+        full_step(sim, ref, w)
+    check(sim, ref, w, TOL_1STEP * 10, err_max)
+
+
 @pytest.mark.parametrize("axis", [0, 1, 2])
 def test_tubes_along_each_axis_with_outflow(pkg, orc, axis):
     for comp in (W.GAS, W.STARS):
@@ -323,7 +346,12 @@ def test_source_from_step_epilogue_equals_fresh_assembly(pkg, orc):
 # isolated Poisson: pruned transforms (power-of-two ny, nz) and the full-cuFFT fallback, against
 # direct summation (the definition, PAPER.md:186 with the boundary reading G3) and the oracle
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("dims", [(4, 4, 4), (16, 8, 32), (8, 32, 4), (10, 16, 8), (6, 4, 64), (10, 12, 6), (8, 6, 8)])
+# the thin grids reach the column transforms the full-size configs run: 256-point (P=8), 512-point
+# (k_colfft<9,4,2>, config 3 at 256^3) and 1024-point columns (k_colfft<10,4,1>, config 5 isolated at 512^3),
+# with their zero-pruned input (nin), the kept-rows remap (nkeep, row 2^P-1) and 4-column tiles
+@pytest.mark.parametrize("dims", [(4, 4, 4), (16, 8, 32), (8, 32, 4), (10, 16, 8), (6, 4, 64), (10, 12, 6), (8, 6, 8),
+                                  (8, 128, 8), (8, 8, 128), (8, 256, 8), (8, 8, 256), (8, 4, 512), (4, 512, 8),
+                                  (12, 256, 4)])
 def test_isolated_poisson_against_direct_summation(pkg, orc, dims):
     nx, ny, nz = dims
     h, G = 0.1, 1.7
