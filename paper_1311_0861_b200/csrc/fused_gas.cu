@@ -1,6 +1,17 @@
 // Fused hydro step of the gas (fused_impl.cuh): footprint of 32 x 16 cells, sixteen Eulerian warps and four
 // Lagrangian warps (640 threads, 96 registers each).
-#define GP_FY 16
+#ifndef GP_GAS_FY
+#define GP_GAS_FY 16
+#define GP_GAS_NDW 12
+#endif
+#ifndef GP_GAS_REG_E
+#define GP_GAS_REG_E 80
+#define GP_GAS_REG_D 56
+#endif
+#define GP_FY GP_GAS_FY
+#define GP_NDW GP_GAS_NDW
+#define GP_REG_E GP_GAS_REG_E
+#define GP_REG_D GP_GAS_REG_D
 #define GP_FUSED_NS fgas
 #define GP_FUSED_GAS 1
 #include "fused_impl.cuh"

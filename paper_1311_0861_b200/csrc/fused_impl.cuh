@@ -20,11 +20,12 @@
 //     wait for U*(j), advect plane j-1 from the four-slot U* ring (4-vertex face velocities as
 //     separable (1/4,1/2,1/4) averages, upwind donor-cell fluxes in coefficient form), write
 //     U^{n+1}(j-1) to HBM and fold its max signal speed.  They also PRODUCE: as soon as all of them
-//     are done with a ring slot, plane j+2 (and Phi(j+3)) is requested into it -- one bulk
-//     asynchronous copy (cp.async.bulk, the TMA engine) per footprint row and field pair, completing
+//     are done with the oldest ring slot, plane j+3 (and Phi(j+4)) is requested into it: one thread
+//     issues one TMA tensor copy (cp.async.bulk.tensor, a 32 x FY x 1 box) per field pair, completing
 //     on an mbarrier with a transaction count; no compute thread issues or waits for a copy
-//     instruction.  Blocks whose x halo is clamped (outflow) or whose rows are not 16-byte aligned
-//     (odd nx) stage cell by cell with cp.async on the same mbarrier.
+//     instruction.  TMA cannot wrap or clamp, so blocks whose footprint reaches over the edge of
+//     the grid (and grids with odd nx, whose rows are not 16-byte aligned) stage cell by cell with
+//     cp.async on the same mbarrier.
 //   * E -> D hand-off: one mbarrier per ring slot ("U*(j) complete"), arrived on by one E thread
 //     after the E barrier.  D -> E: the "landed" mbarrier of the slot.  The E group runs up to two
 //     planes ahead of the D group.  Registers are split between the groups with setmaxnreg.
@@ -33,6 +34,8 @@
 // ghosts are copies of the nearest interior U* (H6), restored in shared memory after E.
 // Phi comes from an array padded by two ghost layers (gp_internal.h, PhiPad), filled by the rule of
 // the Poisson mode, so its staging needs no case analysis.
+#include <cuda.h>
+
 #include "gp_internal.h"
 
 namespace gp {
@@ -43,13 +46,17 @@ namespace GP_FUSED_NS {
 #endif
 constexpr int FX = 32, FY = GP_FY, PL = FX * FY;
 constexpr int TXO = FX - 4, TYO = FY - 4;
+#ifndef GP_NDW
+#define GP_NDW 8
+#endif
 constexpr int NEW = FY;                   // Eulerian warps, one per footprint row
-constexpr int NDW = 4;                    // Lagrangian / producer warps (one warpgroup)
+constexpr int NDW = GP_NDW;               // Lagrangian / producer warps
 constexpr int NTE = NEW * 32, NTD = NDW * 32, NT = NTE + NTD;
 constexpr int DROWS = TYO / NDW;          // output rows per Lagrangian warp
 constexpr int NS = 4;                     // slots of the U* ring
+constexpr int NPHI = 8;                   // slots of the Phi ring
 static_assert(TYO % NDW == 0, "output rows must divide among the Lagrangian warps");
-static_assert(NEW % 4 == 0, "setmaxnreg works on warpgroups of four warps");
+
 // register budgets after the split (0: leave the launch allocation alone)
 #ifndef GP_REG_E
 #define GP_REG_E 0
@@ -57,6 +64,10 @@ static_assert(NEW % 4 == 0, "setmaxnreg works on warpgroups of four warps");
 #ifndef GP_REG_D
 #define GP_REG_D 0
 #endif
+static_assert(GP_REG_E == 0 || (NEW % 4 == 0 && NDW % 4 == 0), "setmaxnreg works on warpgroups of four warps");
+// the block is launched with 65536 / NT registers per thread rounded down to a multiple of 8; the split must fit in
+// that pool, or setmaxnreg.inc waits for ever
+static_assert(GP_REG_E == 0 || NTE * GP_REG_E + NTD * GP_REG_D <= NT * (65536 / NT / 8 * 8), "register split exceeds the block's pool");
 constexpr int BAR_E = 1, BAR_D = 2;       // named barriers (0 is __syncthreads)
 
 // ---- fp64 reciprocal and reciprocal square root: MUFU seed + one cubically convergent step ----
@@ -177,11 +188,12 @@ __device__ __forceinline__ void mbar_arrive_on_cp_async(unsigned long long* b) {
 // order earlier generic-proxy accesses to shared memory before later async-proxy (bulk copy) writes
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// global -> shared bulk copy (TMA engine, SASS UBLKCP): bytes % 16 == 0, both addresses 16-byte aligned;
-// completes bytes on the mbarrier's transaction count
-__device__ __forceinline__ void bulk_g2s(void* smem, const void* gmem, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem)),
-                 "l"(gmem), "r"(bytes), "r"(smem_u32(bar))
+// global -> shared TMA tensor copy of one 3-D box (SASS UTMALDG); completes the box's bytes on the mbarrier's
+// transaction count.  Coordinates are in elements of the map, innermost first.  smem: 128-byte aligned.
+__device__ __forceinline__ void tma_load_3d(void* smem, const CUtensorMap* tm, int c0, int c1, int c2, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     smem_u32(smem)),
+                 "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
                  : "memory");
 }
 __device__ __forceinline__ void cp_async8(double* smem, const double* gmem) {
@@ -239,42 +251,57 @@ __device__ __forceinline__ LagCoef lag_coef(double th64, double wxm, double wxp,
     return c;
 }
 
-// Lagrangian stage of one output cell from three ring slots: rm = plane j-2 (own column only), r0 = plane
-// j-1 (centre and its x, y neighbours), rp = plane j (own column).  Momentum = density * w*, so its
-// update is sum_q (c_q dens_q) w*_q.  NP2 = number of pair planes after P0, P1; LAST1: one more plain
-// plane follows them.  out = (density, momentum x y z, the remaining fields).
+// Lagrangian stage of one output cell from three ring slots, in two parts so that the slot of plane j-2
+// (rm, read at the thread's own column only) can be handed to the staging of a later plane as early as
+// possible: lagrange_lower reads rm, lagrange_rest reads r0 = plane j-1 (centre and its x, y neighbours) and
+// rp = plane j (own column).  Momentum = density * w*, so its update is sum_q (c_q dens_q) w*_q.
+// NP2 = number of pair planes after P0, P1; LAST1: one more plain plane follows them.
+// out = (density, momentum x y z, the remaining fields).
 template <int NP2, bool LAST1>
-__device__ __forceinline__ void lagrange(const double* __restrict__ rm, const double* __restrict__ r0,
-                                         const double* __restrict__ rp, int t, const LagCoef& c,
-                                         double out[4 + 2 * NP2 + (LAST1 ? 1 : 0)]) {
+__device__ __forceinline__ void lagrange_lower(const double* __restrict__ rm, int t, const LagCoef& c,
+                                               double out[4 + 2 * NP2 + (LAST1 ? 1 : 0)]) {
+    const double2 azm = lds2(rm + 2 * t), bzm = lds2(rm + PP + 2 * t);
+    const double dzm = c.zm * azm.x;
+    out[0] = dzm; out[3] = dzm * azm.y; out[1] = dzm * bzm.x; out[2] = dzm * bzm.y;
+#pragma unroll
+    for (int P = 0; P < NP2; ++P) {
+        const double2 ezm = lds2(rm + (2 + P) * PP + 2 * t);
+        out[4 + 2 * P] = c.zm * ezm.x; out[5 + 2 * P] = c.zm * ezm.y;
+    }
+    if (LAST1) out[4 + 2 * NP2] = c.zm * rm[(2 + NP2) * PP + t];
+}
+
+template <int NP2, bool LAST1>
+__device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, const double* __restrict__ rp, int t,
+                                              const LagCoef& c, double out[4 + 2 * NP2 + (LAST1 ? 1 : 0)]) {
     const double2 a0 = lds2(r0 + 2 * t), aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
     const double2 axm = lds2(r0 + 2 * (t - 1)), axp = lds2(r0 + 2 * (t + 1));
-    const double2 azm = lds2(rm + 2 * t), azp = lds2(rp + 2 * t);
+    const double2 azp = lds2(rp + 2 * t);
     const double d0 = c.c0 * a0.x, dxm = c.xm * axm.x, dxp = c.xp * axp.x, dym = c.ym * aym.x, dyp = c.yp * ayp.x,
-                 dzm = c.zm * azm.x, dzp = c.zp * azp.x;
-    out[0] = ((dzm + d0) + (dxm + dxp)) + ((dym + dyp) + dzp);
-    out[3] = fma(dzp, azp.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, fma(d0, a0.y, dzm * azm.y))))));
+                 dzp = c.zp * azp.x;
+    out[0] = ((out[0] + d0) + (dxm + dxp)) + ((dym + dyp) + dzp);
+    out[3] = fma(dzp, azp.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, fma(d0, a0.y, out[3]))))));
     {
         const double2 b0 = lds2(r0 + PP + 2 * t), bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
         const double2 bxm = lds2(r0 + PP + 2 * (t - 1)), bxp = lds2(r0 + PP + 2 * (t + 1));
-        const double2 bzm = lds2(rm + PP + 2 * t), bzp = lds2(rp + PP + 2 * t);
-        out[1] = fma(dzp, bzp.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, fma(d0, b0.x, dzm * bzm.x))))));
-        out[2] = fma(dzp, bzp.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, fma(d0, b0.y, dzm * bzm.y))))));
+        const double2 bzp = lds2(rp + PP + 2 * t);
+        out[1] = fma(dzp, bzp.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, fma(d0, b0.x, out[1]))))));
+        out[2] = fma(dzp, bzp.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, fma(d0, b0.y, out[2]))))));
     }
 #pragma unroll
     for (int P = 0; P < NP2; ++P) {
         const int o = (2 + P) * PP;
         const double2 e0 = lds2(r0 + o + 2 * t), eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
         const double2 exm = lds2(r0 + o + 2 * (t - 1)), exp_ = lds2(r0 + o + 2 * (t + 1));
-        const double2 ezm = lds2(rm + o + 2 * t), ezp = lds2(rp + o + 2 * t);
-        out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, fma(c.c0, e0.x, c.zm * ezm.x))))));
-        out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, fma(c.c0, e0.y, c.zm * ezm.y))))));
+        const double2 ezp = lds2(rp + o + 2 * t);
+        out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, fma(c.c0, e0.x, out[4 + 2 * P]))))));
+        out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, fma(c.c0, e0.y, out[5 + 2 * P]))))));
     }
     if (LAST1) {
         const int o = (2 + NP2) * PP;
         const double e0 = r0[o + t], eym = r0[o + t - FX], eyp = r0[o + t + FX], exm = r0[o + t - 1], exp_ = r0[o + t + 1];
-        const double ezm = rm[o + t], ezp = rp[o + t];
-        out[4 + 2 * NP2] = fma(c.zp, ezp, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, fma(c.c0, e0, c.zm * ezm))))));
+        const double ezp = rp[o + t];
+        out[4 + 2 * NP2] = fma(c.zp, ezp, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, fma(c.c0, e0, out[4 + 2 * NP2]))))));
     }
 }
 
@@ -291,8 +318,11 @@ __device__ __forceinline__ void face_vel_xy(const double* __restrict__ s_tz, int
     wym = b_m + b_0; wyp = b_0 + b_p;
 }
 
+// tensor maps of a launch: the field pairs (then the gas energy) of U, and the padded Phi
 template <int NF>
 struct FusedArgs {
+    alignas(64) CUtensorMap tm[(NF + 1) / 2 + 1];
+    int use_tma;              // the maps are valid (even nx, encode succeeded)
     Geo g;
     const double* U[NF];
     double* Un[NF];
@@ -307,16 +337,14 @@ struct FusedArgs {
 };
 
 // Small per-block tables (shared memory, written once by thread 0).
-struct BlockTab {
+struct alignas(128) BlockTab {
     unsigned long long landed[NS];     // staged plane (+ Phi) has arrived in ring slot s
     unsigned long long ufull[NS];      // U* of ring slot s is complete
     unsigned long long pro;            // the three Phi planes of the prologue have arrived
     long long rowoff[FY];              // nx * (mapped y of footprint row)
     long long phirow[FY];              // pitch * (padded y of footprint row)
-    int seg_dst[3], seg_src[3], seg_len[3], nseg;   // x segments of a footprint row: cells [dst, dst+len) <- x = src ...
     int phi_len;                       // doubles of a Phi row that exist in the padded array
-    int percell;                       // 1: stage cell by cell (cp.async), 0: bulk rows
-    unsigned ubytes, pbytes;           // bytes of one staged plane of the state / of Phi (bulk mode)
+    int percell;                       // 1: stage cell by cell (cp.async), 0: TMA boxes
 };
 
 struct Blk {
@@ -334,63 +362,35 @@ __device__ __forceinline__ Blk make_blk(const Geo& g, int zchunk) {
     return b;
 }
 
-// Bytes per cell of the NPL planes a staged state plane consists of: pairs, then (gas) one plain plane.
-template <int NPAIR, bool LAST1>
-__device__ void build_tab(BlockTab* T, const Geo& g, const PhiPad& phi, const Blk& b) {
-    for (int s = 0; s < NS; ++s) { T->landed[s] = 0; T->ufull[s] = 0; }
+__device__ void build_tab(BlockTab* T, const Geo& g, const PhiPad& phi, const Blk& b, int use_tma) {
     for (int r = 0; r < FY; ++r) {
         T->rowoff[r] = (long long)g.nx * map_safe(b.y0 - 2 + r, g.ny, g.bcy);
         T->phirow[r] = (long long)phi.pitch * min(b.y0 + r, g.ny + 3);
     }
     T->phi_len = min(FX, phi.pitch - b.x0);
-    // x segments: maximal runs of footprint columns whose mapped x is consecutive; columns beyond
-    // x = nx+1 feed no output and are left alone
-    int nseg = 0;
-    bool clamp = false;
-    for (int tx = 0; tx < FX; ++tx) {
-        const int xv = b.x0 - 2 + tx;
-        if (xv > g.nx + 1) break;
-        const int xm = map_safe(xv, g.nx, g.bcx);
-        if (nseg > 0 && T->seg_src[nseg - 1] + T->seg_len[nseg - 1] == xm && T->seg_dst[nseg - 1] + T->seg_len[nseg - 1] == tx) {
-            T->seg_len[nseg - 1]++;
-        } else if (nseg < 3) {
-            T->seg_dst[nseg] = tx; T->seg_src[nseg] = xm; T->seg_len[nseg] = 1; ++nseg;
-        } else {
-            clamp = true;
-        }
-    }
-    for (int s = 0; s < nseg; ++s)
-        if ((T->seg_src[s] | T->seg_len[s] | T->seg_dst[s]) & 1) clamp = true;   // a plain (8-byte) plane needs even runs
-    T->nseg = nseg;
-    T->percell = (clamp || (g.nx & 1)) ? 1 : 0;
-    int cells = 0;
-    for (int s = 0; s < nseg; ++s) cells += T->seg_len[s];
-    T->ubytes = (unsigned)(FY * cells * (16 * NPAIR + (LAST1 ? 8 : 0)));
-    T->pbytes = (unsigned)(FY * T->phi_len * 8);
+    // a TMA box neither wraps nor clamps: the footprint must lie inside the grid
+    const bool inside = b.x0 - 2 >= 0 && b.x0 - 2 + FX <= g.nx && b.y0 - 2 >= 0 && b.y0 - 2 + FY <= g.ny;
+    T->percell = (use_tma && inside) ? 0 : 1;
+#ifdef GP_FORCE_PERCELL
+    T->percell = 1;
+#endif
 }
 
 // Producer (Lagrangian warps): request plane kz of the state into ring slot `dst` (layout above: NPAIR pair
-// planes, then one plain plane if LAST1).  Bulk mode: lanes of warp 0 share the FY*planes*segments row copies.
+// planes, then one plain plane if LAST1).  TMA mode: thread 0 of the group issues one box per plane.
 template <int NPAIR, bool LAST1, int NF>
 __device__ __forceinline__ void stage_state(const FusedArgs<NF>& a, const BlockTab* T, const Blk& b, double* dst, int kz,
                                             unsigned long long* bar, int dtid) {
     const Geo& g = a.g;
-    const long long zoff = (long long)map_safe(kz, g.nz, g.bcz) * g.nx * g.ny;
-    constexpr int NPLN = NPAIR + (LAST1 ? 1 : 0);
+    const int zm = map_safe(kz, g.nz, g.bcz);
     if (!T->percell) {
-        if (dtid < 32) {
-            const int n = FY * NPLN * T->nseg;
-            for (int i = dtid; i < n; i += 32) {
-                const int row = i % FY, q = i / FY, P = q % NPLN, s = q / NPLN;
-                const long long cell = zoff + T->rowoff[row] + T->seg_src[s];
-                const int tcell = row * FX + T->seg_dst[s];
-                if (LAST1 && P == NPAIR)
-                    bulk_g2s(dst + NPAIR * PP + tcell, a.U[2 * NPAIR] + cell, 8u * T->seg_len[s], bar);
-                else
-                    bulk_g2s(dst + P * PP + 2 * tcell, a.U[2 * P] + BSTR * cell, 16u * T->seg_len[s], bar);
-            }
+        if (dtid == 0) {
+#pragma unroll
+            for (int P = 0; P < NPAIR; ++P) tma_load_3d(dst + P * PP, &a.tm[P], 2 * (b.x0 - 2), b.y0 - 2, zm, bar);
+            if (LAST1) tma_load_3d(dst + NPAIR * PP, &a.tm[NPAIR], b.x0 - 2, b.y0 - 2, zm, bar);
         }
     } else {
+        const long long zoff = (long long)zm * g.nx * g.ny;
         for (int c = dtid; c < PL; c += NTD) {
             const int row = c / FX, tx = c % FX;
             const long long cell = zoff + T->rowoff[row] + map_safe(b.x0 - 2 + tx, g.nx, g.bcx);
@@ -406,10 +406,10 @@ template <int NF>
 __device__ __forceinline__ void stage_phi(const FusedArgs<NF>& a, const BlockTab* T, const Blk& b, double* dst, int kz,
                                           unsigned long long* bar, int dtid) {
     const PhiPad& p = a.phi;
-    const double* src = p.p + (long long)p.pitch * p.py * (kz + 2) + b.x0;
     if (!T->percell) {
-        if (dtid < FY) bulk_g2s(dst + dtid * FX, src + T->phirow[dtid], 8u * T->phi_len, bar);
+        if (dtid == 0) tma_load_3d(dst, &a.tm[(NF + 1) / 2], b.x0, b.y0, kz + 2, bar);
     } else {
+        const double* src = p.p + (long long)p.pitch * p.py * (kz + 2) + b.x0;
         for (int c = dtid; c < PL; c += NTD) {
             const int row = c / FX, tx = c % FX;
             cp_async8(dst + c, src + T->phirow[row] + min(tx, T->phi_len - 1));
@@ -482,60 +482,30 @@ struct LagRows {
     int bad;
 };
 
-// One plane of the Lagrangian warps' loop (see the header).  Traits TR supply the component's layout.
-template <class TR, int NF>
-__device__ __forceinline__ void lag_plane(const FusedArgs<NF>& a, const BlockTab* T, const Blk& b, double* ring, double* tz,
-                                          LagRows& L, int j, double th, int dw, int lane) {
-    const Geo& g = a.g;
-    const bool zout = g.bcz == GP_BC_OUTFLOW;
-    const bool bot_dup = zout && j == 0;
-    const bool do_out = j - 1 >= b.z0;
-    const bool do_wzp = j >= b.z0;
-    const int it = j - (b.z0 - 1);
-    const double* rs = ring + (it & 3) * TR::SLOT;
-    const double* r0 = ring + ((it + 3) & 3) * TR::SLOT;
-    const double* rm = ring + ((it + 2) & 3) * TR::SLOT;
-    const double* tzj = tz + (it & 1) * PP;
-    const size_t nxny = (size_t)g.nx * g.ny;
-#pragma unroll
-    for (int q = 0; q < DROWS; ++q) {
-        const int ty = 2 + dw + NDW * q;
-        const int t = ty * FX + lane;
-        const double Sz_new = sum9_wz(rs, t);             // 16 x
-        if (bot_dup) L.Sz_prev[q] = Sz_new;
-        if (do_wzp) {
-            const double wzp = L.Sz_prev[q] + Sz_new;      // 32 x face velocity between planes j-1 and j
-            if (do_out) {
-                double wxm, wxp, wym, wyp;
-                face_vel_xy(tzj, t, wxm, wxp, wym, wyp);
-                const LagCoef lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, L.wzp_prev[q], wzp);
-                const int xv = b.x0 - 2 + lane, yv = b.y0 - 2 + ty;
-                const bool is_out = lane >= 2 && lane <= FX - 3 && xv < g.nx && yv < g.ny;
-                const size_t off = (size_t)xv + (size_t)g.nx * yv + (size_t)(j - 1) * nxny;
-                double out[NF];
-                lagrange<TR::NP2, TR::LAST1>(rm, r0, rs, t, lc, out);
-                if (is_out) TR::emit(a, off, out, L.smax, L.bad);
-            }
-            L.wzp_prev[q] = wzp;
-        }
-        L.Sz_prev[q] = Sz_new;
-    }
-}
-
-// The Lagrangian warps' whole loop, prologue included.
+// The Lagrangian warps' whole loop, prologue included (see the header).  Traits TR supply the component's
+// layout.  Per plane j (it = j - (z0-1)): wait for U*(j); face velocities and upwind coefficients of the warp's
+// rows; the part of the update that reads ring slot it+2 (plane j-2, own column); hand that slot over: it takes
+// the staged plane j+3 (consumed by E(j+2), two planes ahead of the Eulerian warps); then the rest.
 template <class TR, int NF>
 __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, const Blk& b, double* ring, double* tz,
                                           double* phir, double th, LagRows& L) {
+    const Geo& g = a.g;
     const int dtid = threadIdx.x - NTE, dw = dtid >> 5, lane = dtid & 31;
     const int j0 = b.z0 - 1;
     const bool bulk = !T->percell;
+    constexpr unsigned UBYTES = PL * (16 * TR::NPAIR + (TR::LAST1 ? 8 : 0)), PBYTES = PL * 8;   // one staged plane: state, Phi
+    const bool zout = g.bcz == GP_BC_OUTFLOW;
+    const size_t nxny = (size_t)g.nx * g.ny;
 #pragma unroll
     for (int q = 0; q < DROWS; ++q) L.Sz_prev[q] = L.wzp_prev[q] = 0.0;
     L.smax = 0.0; L.bad = 0;
-    // prologue: Phi(z0-2 .. z0) for the first B and C, then the bundle of ring slot 0: U(z0), Phi(z0+1)
+    // prologue: Phi(z0-2 .. z0) for the first B and C, then the bundles of ring slots 0 and 1:
+    // (U(z0), Phi(z0+1)) for E(z0-1) and (U(z0+1), Phi(z0+2)) for E(z0)
+    const bool phi2 = b.z0 + 1 <= b.z1;       // C(z0+1) exists and needs Phi(z0+2)
     if (bulk && dtid == 0) {
-        mbar_arrive_expect_tx(&T->pro, 3 * T->pbytes);
-        mbar_arrive_expect_tx(&T->landed[0], T->ubytes + T->pbytes);
+        mbar_arrive_expect_tx(&T->pro, 3 * PBYTES);
+        mbar_arrive_expect_tx(&T->landed[0], UBYTES + PBYTES);
+        mbar_arrive_expect_tx(&T->landed[1], UBYTES + (phi2 ? PBYTES : 0u));
     }
     __syncwarp();
     for (int k = 0; k < 3; ++k) stage_phi(a, T, b, phir + k * PL, b.z0 - 2 + k, &T->pro, dtid);
@@ -543,44 +513,88 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
     stage_state<TR::NPAIR, TR::LAST1>(a, T, b, ring, b.z0, &T->landed[0], dtid);
     stage_phi(a, T, b, phir + 3 * PL, b.z0 + 1, &T->landed[0], dtid);
     if (!bulk) mbar_arrive_on_cp_async(&T->landed[0]);
+    stage_state<TR::NPAIR, TR::LAST1>(a, T, b, ring + TR::SLOT, b.z0 + 1, &T->landed[1], dtid);
+    if (phi2) stage_phi(a, T, b, phir + 4 * PL, b.z0 + 2, &T->landed[1], dtid);
+    if (!bulk) mbar_arrive_on_cp_async(&T->landed[1]);
 
     for (int j = j0; j <= b.z1; ++j) {
         const int it = j - j0;
-        bar_sync(BAR_D, NTD);                 // every Lagrangian warp is done with plane j-1: slot it+1 is free
-        const bool more = j + 1 <= b.z1;      // E(j+1) exists and needs U(j+2)
-        const bool more_phi = j + 2 <= b.z1;  // C(j+2) exists and needs Phi(j+3)
-        unsigned long long* land = &T->landed[(it + 1) & 3];
-        if (more) {
-            if (bulk) {
-                fence_proxy_async();
-                if (dtid == 0) mbar_arrive_expect_tx(land, T->ubytes + (more_phi ? T->pbytes : 0u));
-                __syncwarp();
+        const bool bot_dup = zout && j == 0;
+        const bool do_out = j - 1 >= b.z0;
+        const bool do_wzp = j >= b.z0;
+        const double* rs = ring + (it & 3) * TR::SLOT;
+        const double* r0 = ring + ((it + 3) & 3) * TR::SLOT;
+        const double* rm = ring + ((it + 2) & 3) * TR::SLOT;
+        const double* tzj = tz + (it & 1) * PP;
+        mbar_wait(&T->ufull[it & 3], (it >> 2) & 1);      // U*(j) complete
+
+        const bool more = j + 2 <= b.z1;          // E(j+2) exists and needs U(j+3)
+        const bool more_phi = j + 3 <= b.z1;      // C(j+3) exists and needs Phi(j+4)
+#pragma unroll
+        for (int q = 0; q < DROWS; ++q) {
+            const int ty = 2 + dw + NDW * q;
+            const int t = ty * FX + lane;
+            LagCoef lc;
+            double out[NF];
+            bool emit = false;
+            const double Sz_new = sum9_wz(rs, t);             // 16 x
+            if (bot_dup) L.Sz_prev[q] = Sz_new;
+            if (do_wzp) {
+                const double wzp = L.Sz_prev[q] + Sz_new;      // 32 x face velocity between planes j-1 and j
+                if (do_out) {
+                    double wxm, wxp, wym, wyp;
+                    face_vel_xy(tzj, t, wxm, wxp, wym, wyp);
+                    lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, L.wzp_prev[q], wzp);
+                    lagrange_lower<TR::NP2, TR::LAST1>(rm, t, lc, out);
+                    emit = true;
+                }
+                L.wzp_prev[q] = wzp;
             }
-            stage_state<TR::NPAIR, TR::LAST1>(a, T, b, ring + ((it + 1) & 3) * TR::SLOT, j + 2, land, dtid);
-        }
-        mbar_wait(&T->ufull[it & 3], (it >> 2) & 1);      // U*(j) complete (and C(j) done with Phi(j-1))
-        if (more) {
-            if (more_phi) {
+            L.Sz_prev[q] = Sz_new;
+
+            // After the last row's lower part ring slot it+2 (plane j-2) is no longer needed by this warp; when
+            // that holds for all of them it takes the bundle of plane j+2: U(j+3) and Phi(j+4)
+            if (q == DROWS - 1 && more) {
+                unsigned long long* land = &T->landed[(it + 2) & 3];
+                double* dst = ring + ((it + 2) & 3) * TR::SLOT;
+                double* pdst = phir + ((it + 5) & (NPHI - 1)) * PL;
                 if (bulk) fence_proxy_async();
-                stage_phi(a, T, b, phir + ((it + 4) & 3) * PL, j + 3, land, dtid);
+                bar_sync(BAR_D, NTD);
+                if (bulk) {
+                    if (dtid == 0) {
+                        mbar_arrive_expect_tx(land, UBYTES + (more_phi ? PBYTES : 0u));
+                        stage_state<TR::NPAIR, TR::LAST1>(a, T, b, dst, j + 3, land, dtid);
+                        if (more_phi) stage_phi(a, T, b, pdst, j + 4, land, dtid);
+                    }
+                } else {
+                    stage_state<TR::NPAIR, TR::LAST1>(a, T, b, dst, j + 3, land, dtid);
+                    if (more_phi) stage_phi(a, T, b, pdst, j + 4, land, dtid);
+                    mbar_arrive_on_cp_async(land);
+                }
             }
-            if (!bulk) mbar_arrive_on_cp_async(land);
+
+            if (emit) {
+                lagrange_rest<TR::NP2, TR::LAST1>(r0, rs, t, lc, out);
+                const int xv = b.x0 - 2 + lane, yv = b.y0 - 2 + ty;
+                const bool is_out = lane >= 2 && lane <= FX - 3 && xv < g.nx && yv < g.ny;
+                const size_t off = (size_t)xv + (size_t)g.nx * yv + (size_t)(j - 1) * nxny;
+                if (is_out) TR::emit(a, off, out, L.smax, L.bad);
+            }
         }
-        lag_plane<TR>(a, T, b, ring, tz, L, j, th, dw, lane);
     }
 }
 
 #ifdef GP_FUSED_GAS
 // =================================================================================================
 // Gas: fields rho, mx, my, mz, E.
-// Shared planes (of PL doubles): (rho,p) pair 2, vx 1, vy 1, Phi ring 4, y-flux (P,PV) pair 2,
-// U* ring 4 x (2 pair planes + 1 plain) = 20, z-averaged (w*_x,w*_y) pair 2 x 2 = 4  ->  34 planes.
+// Shared planes (of PL doubles): (rho,p) pair 2, vx 1, vy 1, Phi ring 8, y-flux (P,PV) pair 2,
+// U* ring 4 x (2 pair planes + 1 plain) = 20, z-averaged (w*_x,w*_y) pair 2 x 2 = 4  ->  38 planes.
 // =================================================================================================
 struct GasTraits {
     static constexpr int NPAIR = 2, NP2 = 0;
     static constexpr bool LAST1 = true;
     static constexpr int SLOT = 2 * PP + PL;
-    static constexpr int PLANES = 2 + 1 + 1 + 4 + 2 + NS * 5 + 4;
+    static constexpr int PLANES = 2 + 1 + 1 + NPHI + 2 + NS * 5 + 4;
     __device__ static __forceinline__ void emit(const FusedArgs<NGAS>& a, size_t off, const double out[NGAS], double& smax, int& bad) {
         double n_other = 0.0;
         if (a.src_in) n_other = a.src_in[BSTR * off];
@@ -622,7 +636,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     const bool bot_dup = !ST && zout && j == 0;
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
-    const double* ph0 = S.phi + ((it + 1) & 3) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
+    const double* ph0 = S.phi + ((it + 1) & (NPHI - 1)) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
 
     // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
     // that the two solvers interleave.  Row FY-1 has no row above it; its faces are never used.
@@ -675,7 +689,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
             const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
             dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y; Es = rq[2 * PP + t];
         } else {
-            const double gz = (S.phi[((it + 2) & 3) * PL + t] - S.phi[(it & 3) * PL + t]) * inv2h;
+            const double gz = (S.phi[((it + 2) & (NPHI - 1)) * PL + t] - S.phi[(it & (NPHI - 1)) * PL + t]) * inv2h;
             const double trg = tau * c.rho * gz;
             const double mz = c.rho * c.vz;
             const double mzs = c.amz - th2 * Pz - trg;
@@ -718,18 +732,18 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
 }
 
 __global__ void __launch_bounds__(NT, 1)
-k_fused_gas(FusedArgs<NGAS> a) {
-    extern __shared__ double2 sm2[];
-    BlockTab* T = reinterpret_cast<BlockTab*>(sm2);
-    double* sm = reinterpret_cast<double*>(sm2) + (sizeof(BlockTab) + 15) / 16 * 2;
+k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
+    extern __shared__ __align__(128) unsigned char smraw[];
+    BlockTab* T = reinterpret_cast<BlockTab*>(smraw);
+    double* sm = reinterpret_cast<double*>(smraw + sizeof(BlockTab));
     GasShared S;
-    S.rp = sm; S.vx = sm + 2 * PL; S.vy = sm + 3 * PL; S.phi = sm + 4 * PL; S.fy = sm + 8 * PL;
-    S.ring = sm + 10 * PL; S.tz = S.ring + NS * GasTraits::SLOT;
+    S.rp = sm; S.vx = sm + 2 * PL; S.vy = sm + 3 * PL; S.phi = sm + 4 * PL; S.fy = S.phi + NPHI * PL;
+    S.ring = S.fy + 2 * PL; S.tz = S.ring + NS * GasTraits::SLOT;
 
     const Geo& g = a.g;
     const Blk b = make_blk(g, a.zchunk);
     if (threadIdx.x == 0) {
-        build_tab<GasTraits::NPAIR, GasTraits::LAST1>(T, g, a.phi, b);
+        build_tab(T, g, a.phi, b, a.use_tma);
         const unsigned cnt = T->percell ? NTD : 1;
         for (int s = 0; s < NS; ++s) { mbar_init(&T->landed[s], cnt); mbar_init(&T->ufull[s], 1); }
         mbar_init(&T->pro, cnt);
@@ -792,14 +806,14 @@ k_fused_gas(FusedArgs<NGAS> a) {
 // =================================================================================================
 // Collisionless component: fields n, nu (3), nE_ij (6: xx xy xz yy yz zz).
 // Shared planes (of PL doubles): primitives (n,ux) (uy,uz) (Pxx,Pxz) (Pyy,Pyz) pairs 8 + Pxy 1,
-// Phi ring 4, y-flux (Ps0,Ps1) (Ps2,EF0) (EF1,EF2) (EF3,EF4) pairs 8 + EF5 1, U* ring 4 x 5 pair planes = 40,
-// z-averaged (w*_x,w*_y) pair 2 x 2 = 4  ->  66 planes (198 KB at FY = 12).
+// Phi ring 8, y-flux (Ps0,Ps1) (Ps2,EF0) (EF1,EF2) (EF3,EF4) pairs 8 + EF5 1, U* ring 4 x 5 pair planes = 40,
+// z-averaged (w*_x,w*_y) pair 2 x 2 = 4  ->  70 planes (210 KB at FY = 12).
 // =================================================================================================
 struct BmeTraits {
     static constexpr int NPAIR = 5, NP2 = 3;
     static constexpr bool LAST1 = false;
     static constexpr int SLOT = 5 * PP;
-    static constexpr int PLANES = 9 + 4 + 9 + NS * 10 + 4;
+    static constexpr int PLANES = 9 + NPHI + 9 + NS * 10 + 4;
     __device__ static __forceinline__ void emit(const FusedArgs<NBME>& a, size_t off, const double out[NBME], double& smax, int& bad) {
 #pragma unroll
         for (int P = 0; P < NBME / 2; ++P)
@@ -840,7 +854,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     const bool bot_dup = !ST && zout && j == 0;
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
-    const double* ph0 = S.phi + ((it + 1) & 3) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
+    const double* ph0 = S.phi + ((it + 1) & (NPHI - 1)) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
 
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
     // dependent chains interleave; rows 0 and FY-1 (halo rows whose results are never used) run them on
@@ -880,7 +894,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         c.acc[3] -= th4 * (EFy[0] - l1.y); c.acc[4] -= th4 * (EFy[1] - l2.x); c.acc[5] -= th4 * (EFy[2] - l2.y);
         c.acc[6] -= th4 * (EFy[3] - l3.x); c.acc[7] -= th4 * (EFy[4] - l3.y); c.acc[8] -= th4 * (EFy[5] - l4);
         // gravity (reading G5): -tau n g_i and -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
-        const double gr[3] = {gx, gy, (S.phi[((it + 2) & 3) * PL + t] - S.phi[(it & 3) * PL + t]) * inv2h};
+        const double gr[3] = {gx, gy, (S.phi[((it + 2) & (NPHI - 1)) * PL + t] - S.phi[(it & (NPHI - 1)) * PL + t]) * inv2h};
         double uc[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], c.u[d]);
@@ -974,18 +988,18 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
 }
 
 __global__ void __launch_bounds__(NT, 1)
-k_fused_bme(FusedArgs<NBME> a) {
-    extern __shared__ double2 sm2[];
-    BlockTab* T = reinterpret_cast<BlockTab*>(sm2);
-    double* sm = reinterpret_cast<double*>(sm2) + (sizeof(BlockTab) + 15) / 16 * 2;
+k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
+    extern __shared__ __align__(128) unsigned char smraw[];
+    BlockTab* T = reinterpret_cast<BlockTab*>(smraw);
+    double* sm = reinterpret_cast<double*>(smraw + sizeof(BlockTab));
     BmeShared S;
     S.nu = sm; S.uu = sm + 2 * PL; S.px = sm + 4 * PL; S.py = sm + 6 * PL; S.pxy = sm + 8 * PL; S.phi = sm + 9 * PL;
-    S.fy = sm + 13 * PL; S.ring = sm + 22 * PL; S.tz = S.ring + NS * BmeTraits::SLOT;
+    S.fy = S.phi + NPHI * PL; S.ring = S.fy + 9 * PL; S.tz = S.ring + NS * BmeTraits::SLOT;
 
     const Geo& g = a.g;
     const Blk b = make_blk(g, a.zchunk);
     if (threadIdx.x == 0) {
-        build_tab<BmeTraits::NPAIR, BmeTraits::LAST1>(T, g, a.phi, b);
+        build_tab(T, g, a.phi, b, a.use_tma);
         const unsigned cnt = T->percell ? NTD : 1;
         for (int s = 0; s < NS; ++s) { mbar_init(&T->landed[s], cnt); mbar_init(&T->ufull[s], 1); }
         mbar_init(&T->pro, cnt);
@@ -1073,6 +1087,31 @@ static int pick_zchunk(const gp_ctx* c, int tiles_xy) {
     return best;
 }
 
+// Tensor maps of one launch (host side, a few microseconds): field pairs as rows of 2 nx doubles, the gas energy and
+// the padded Phi as rows of doubles; boxes of one footprint plane.  Returns false if TMA cannot describe the grid
+// (odd nx: rows not 16-byte aligned) or the driver entry point is missing; the kernel then stages cell by cell.
+typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static bool encode_map(CUtensorMap* tm, const void* base, size_t row_doubles, size_t ny, size_t nz, unsigned box_doubles) {
+    static EncodeTiled enc = nullptr;
+    static bool looked = false;
+    if (!looked) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            enc = (EncodeTiled)fn;
+        looked = true;
+    }
+    if (!enc || (row_doubles & 1)) return false;
+    const cuuint64_t dims[3] = {row_doubles, ny, nz};
+    const cuuint64_t strides[2] = {row_doubles * sizeof(double), row_doubles * ny * sizeof(double)};
+    const cuuint32_t box[3] = {box_doubles, (cuuint32_t)FY, 1}, estr[3] = {1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int NF, class K>
 static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, double dt, const double* d_dt,
                           const double* src_in = nullptr, double* src_out = nullptr) {
@@ -1081,12 +1120,17 @@ static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, doub
     a.g = Geo{c->g.nx, c->g.ny, c->g.nz, c->bc.x, c->bc.y, c->bc.z};
     for (int f = 0; f < NF; ++f) { a.U[f] = c->U[f0 + f]; a.Un[f] = c->Us[f0 + f]; }
     a.phi = phipad_of(c);
+    bool ok = true;
+    for (int P = 0; P < NF / 2; ++P) ok = ok && encode_map(&a.tm[P], a.U[2 * P], 2 * (size_t)c->g.nx, c->g.ny, c->g.nz, 2 * FX);
+    if (NF & 1) ok = ok && encode_map(&a.tm[NF / 2], a.U[NF - 1], c->g.nx, c->g.ny, c->g.nz, FX);
+    ok = ok && encode_map(&a.tm[(NF + 1) / 2], a.phi.p, a.phi.pitch, a.phi.py, (size_t)c->g.nz + 4, FX);
+    a.use_tma = ok ? 1 : 0;
     a.h = c->g.h; a.gamma = c->gamma; a.dt_val = dt; a.dt_ptr = d_dt;
     a.smax_bits = c->d_smax_next; a.flag = c->d_flag_next;
     const int tx = (c->g.nx + TXO - 1) / TXO, ty = (c->g.ny + TYO - 1) / TYO;
     a.zchunk = pick_zchunk(c, tx * ty);
     const int tz = (c->g.nz + a.zchunk - 1) / a.zchunk;
-    const size_t smem = (size_t)planes * PL * sizeof(double) + (sizeof(BlockTab) + 15) / 16 * 16;
+    const size_t smem = (size_t)planes * PL * sizeof(double) + sizeof(BlockTab);
     // the opt-in is per device and cheap: set it on every launch (a context may live on any device)
     GP_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     tic(c, kid);
