@@ -5,8 +5,8 @@
 #define GP_GAS_NDW 12
 #endif
 #ifndef GP_GAS_REG_E
-#define GP_GAS_REG_E 80
-#define GP_GAS_REG_D 56
+#define GP_GAS_REG_E 72
+#define GP_GAS_REG_D 64
 #endif
 #define GP_FY GP_GAS_FY
 #define GP_NDW GP_GAS_NDW

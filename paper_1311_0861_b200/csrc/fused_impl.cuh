@@ -15,7 +15,7 @@
 //          primitives, z face (j, j+1), complete U*(j) and write it (density, w* = momentum*/
 //          density, remaining fields) over the staged data -- U* never goes to HBM -- and publish
 //          the primitives of plane j+1 for the next B.
-//     Two named barriers (E warps only) per plane, after B and after E.
+//     Rows synchronise with their two neighbours only (named barriers of 64 threads, row_arrive / row_wait).
 //   * 4 Lagrangian warps ("D", one warpgroup; each serves (FY-4)/4 output rows).  Per plane j they
 //     wait for U*(j), advect plane j-1 from the four-slot U* ring (4-vertex face velocities as
 //     separable (1/4,1/2,1/4) averages, upwind donor-cell fluxes in coefficient form), write
@@ -68,7 +68,6 @@ static_assert(GP_REG_E == 0 || (NEW % 4 == 0 && NDW % 4 == 0), "setmaxnreg works
 // the block is launched with 65536 / NT registers per thread rounded down to a multiple of 8; the split must fit in
 // that pool, or setmaxnreg.inc waits for ever
 static_assert(GP_REG_E == 0 || NTE * GP_REG_E + NTD * GP_REG_D <= NT * (65536 / NT / 8 * 8), "register split exceeds the block's pool");
-constexpr int BAR_E = 1, BAR_D = 2;       // named barriers (0 is __syncthreads)
 
 // ---- fp64 reciprocal and reciprocal square root: MUFU seed + one cubically convergent step ----
 // seed relative error <= 2^-20  ->  after the step <= ~2^-59; final rounding ~1 ulp.
@@ -159,8 +158,6 @@ __device__ __forceinline__ double2 lds2(const double* p) { return *reinterpret_c
 __device__ __forceinline__ void sts2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-__device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
-
 __device__ __forceinline__ void mbar_init(unsigned long long* b, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
@@ -180,6 +177,22 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
         "bra W_%=;\n\t"
         "D_%=:\n\t}" ::"r"(smem_u32(b)), "r"(parity)
         : "memory");
+}
+// Neighbouring Eulerian warps (footprint rows r, r+1) hand data to each other through two mbarriers per row, one
+// arrival (lane 0 of the producing row) per plane, phase parity = plane parity: yrdy[r] "the y fluxes of row r are
+// written" (row r+1 waits before stage C) and prdy[r] "the primitives of the next plane of row r are published" (row
+// r-1 waits before its next stage B).  Each also orders the overwrite that follows it: row r+1 publishes new primitives
+// only after row r has read the old ones, row r rewrites its y fluxes only after row r+1 has read them.  No
+// block-wide barrier is left in the Eulerian group.
+__device__ __forceinline__ void row_arrive(unsigned long long* b) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(b);
+}
+// barrier among the warps of one group: one lane per warp arrives, everybody waits for the phase
+__device__ __forceinline__ void group_sync(unsigned long long* b, unsigned parity) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(b);
+    mbar_wait(b, parity);
 }
 // the arrival is triggered when every cp.async this thread issued before has completed
 __device__ __forceinline__ void mbar_arrive_on_cp_async(unsigned long long* b) {
@@ -251,58 +264,41 @@ __device__ __forceinline__ LagCoef lag_coef(double th64, double wxm, double wxp,
     return c;
 }
 
-// Lagrangian stage of one output cell from three ring slots, in two parts so that the slot of plane j-2
-// (rm, read at the thread's own column only) can be handed to the staging of a later plane as early as
-// possible: lagrange_lower reads rm, lagrange_rest reads r0 = plane j-1 (centre and its x, y neighbours) and
-// rp = plane j (own column).  Momentum = density * w*, so its update is sum_q (c_q dens_q) w*_q.
-// NP2 = number of pair planes after P0, P1; LAST1: one more plain plane follows them.
-// out = (density, momentum x y z, the remaining fields).
-template <int NP2, bool LAST1>
-__device__ __forceinline__ void lagrange_lower(const double* __restrict__ rm, int t, const LagCoef& c,
-                                               double out[4 + 2 * NP2 + (LAST1 ? 1 : 0)]) {
-    const double2 azm = lds2(rm + 2 * t), bzm = lds2(rm + PP + 2 * t);
-    const double dzm = c.zm * azm.x;
-    out[0] = dzm; out[3] = dzm * azm.y; out[1] = dzm * bzm.x; out[2] = dzm * bzm.y;
+// Lagrangian stage of one output cell, neighbour by neighbour: out += c_q * U*_q for one neighbour cell tq of
+// ring slot r (PAPER.md:124, 128 in the coefficient form above).  Momentum = density * w*, so its update is
+// (c_q dens_q) w*_q.  NP2 = number of pair planes after P0, P1; LAST1: one more plain plane follows them.
+// out = (density, momentum x y z, the remaining fields).  INIT: out = ... instead of out += ...
+// An upwind scheme reads a neighbour only where the flow comes from it: c_q = 0 on the downwind side, and when
+// that holds for every output lane of the warp the caller skips the neighbour altogether (lag_needed).
+template <int NP2, bool LAST1, bool INIT>
+__device__ __forceinline__ void lagrange_add(const double* __restrict__ r, int tq, double cq,
+                                             double out[4 + 2 * NP2 + (LAST1 ? 1 : 0)]) {
+    const double2 a = lds2(r + 2 * tq), b = lds2(r + PP + 2 * tq);
+    double2 e[NP2 > 0 ? NP2 : 1];
 #pragma unroll
-    for (int P = 0; P < NP2; ++P) {
-        const double2 ezm = lds2(rm + (2 + P) * PP + 2 * t);
-        out[4 + 2 * P] = c.zm * ezm.x; out[5 + 2 * P] = c.zm * ezm.y;
+    for (int P = 0; P < NP2; ++P) e[P] = lds2(r + (2 + P) * PP + 2 * tq);
+    double el = 0.0;
+    if (LAST1) el = r[(2 + NP2) * PP + tq];
+    const double d = cq * a.x;
+    if (INIT) {
+        out[0] = d; out[3] = d * a.y; out[1] = d * b.x; out[2] = d * b.y;
+#pragma unroll
+        for (int P = 0; P < NP2; ++P) { out[4 + 2 * P] = cq * e[P].x; out[5 + 2 * P] = cq * e[P].y; }
+        if (LAST1) out[4 + 2 * NP2] = cq * el;
+    } else {
+        out[0] += d; out[3] = fma(d, a.y, out[3]); out[1] = fma(d, b.x, out[1]); out[2] = fma(d, b.y, out[2]);
+#pragma unroll
+        for (int P = 0; P < NP2; ++P) { out[4 + 2 * P] = fma(cq, e[P].x, out[4 + 2 * P]); out[5 + 2 * P] = fma(cq, e[P].y, out[5 + 2 * P]); }
+        if (LAST1) out[4 + 2 * NP2] = fma(cq, el, out[4 + 2 * NP2]);
     }
-    if (LAST1) out[4 + 2 * NP2] = c.zm * rm[(2 + NP2) * PP + t];
 }
-
-template <int NP2, bool LAST1>
-__device__ __forceinline__ void lagrange_rest(const double* __restrict__ r0, const double* __restrict__ rp, int t,
-                                              const LagCoef& c, double out[4 + 2 * NP2 + (LAST1 ? 1 : 0)]) {
-    const double2 a0 = lds2(r0 + 2 * t), aym = lds2(r0 + 2 * (t - FX)), ayp = lds2(r0 + 2 * (t + FX));
-    const double2 axm = lds2(r0 + 2 * (t - 1)), axp = lds2(r0 + 2 * (t + 1));
-    const double2 azp = lds2(rp + 2 * t);
-    const double d0 = c.c0 * a0.x, dxm = c.xm * axm.x, dxp = c.xp * axp.x, dym = c.ym * aym.x, dyp = c.yp * ayp.x,
-                 dzp = c.zp * azp.x;
-    out[0] = ((out[0] + d0) + (dxm + dxp)) + ((dym + dyp) + dzp);
-    out[3] = fma(dzp, azp.y, fma(dyp, ayp.y, fma(dym, aym.y, fma(dxp, axp.y, fma(dxm, axm.y, fma(d0, a0.y, out[3]))))));
-    {
-        const double2 b0 = lds2(r0 + PP + 2 * t), bym = lds2(r0 + PP + 2 * (t - FX)), byp = lds2(r0 + PP + 2 * (t + FX));
-        const double2 bxm = lds2(r0 + PP + 2 * (t - 1)), bxp = lds2(r0 + PP + 2 * (t + 1));
-        const double2 bzp = lds2(rp + PP + 2 * t);
-        out[1] = fma(dzp, bzp.x, fma(dyp, byp.x, fma(dym, bym.x, fma(dxp, bxp.x, fma(dxm, bxm.x, fma(d0, b0.x, out[1]))))));
-        out[2] = fma(dzp, bzp.y, fma(dyp, byp.y, fma(dym, bym.y, fma(dxp, bxp.y, fma(dxm, bxm.y, fma(d0, b0.y, out[2]))))));
-    }
-#pragma unroll
-    for (int P = 0; P < NP2; ++P) {
-        const int o = (2 + P) * PP;
-        const double2 e0 = lds2(r0 + o + 2 * t), eym = lds2(r0 + o + 2 * (t - FX)), eyp = lds2(r0 + o + 2 * (t + FX));
-        const double2 exm = lds2(r0 + o + 2 * (t - 1)), exp_ = lds2(r0 + o + 2 * (t + 1));
-        const double2 ezp = lds2(rp + o + 2 * t);
-        out[4 + 2 * P] = fma(c.zp, ezp.x, fma(c.yp, eyp.x, fma(c.ym, eym.x, fma(c.xp, exp_.x, fma(c.xm, exm.x, fma(c.c0, e0.x, out[4 + 2 * P]))))));
-        out[5 + 2 * P] = fma(c.zp, ezp.y, fma(c.yp, eyp.y, fma(c.ym, eym.y, fma(c.xp, exp_.y, fma(c.xm, exm.y, fma(c.c0, e0.y, out[5 + 2 * P]))))));
-    }
-    if (LAST1) {
-        const int o = (2 + NP2) * PP;
-        const double e0 = r0[o + t], eym = r0[o + t - FX], eyp = r0[o + t + FX], exm = r0[o + t - 1], exp_ = r0[o + t + 1];
-        const double ezp = rp[o + t];
-        out[4 + 2 * NP2] = fma(c.zp, ezp, fma(c.yp, eyp, fma(c.ym, eym, fma(c.xp, exp_, fma(c.xm, exm, fma(c.c0, e0, out[4 + 2 * NP2]))))));
-    }
+// does any output lane of the warp take anything from this neighbour?
+__device__ __forceinline__ bool lag_needed(double cq, bool lane_out) {
+#ifdef GP_NO_UPWIND_SKIP
+    return true;
+#else
+    return __any_sync(FULL, lane_out && cq != 0.0) != 0;
+#endif
 }
 
 // 32 x the face velocities of one output cell (reading G2) from the z-summed (4 x averaged) w*_x,
@@ -341,6 +337,8 @@ struct alignas(128) BlockTab {
     unsigned long long landed[NS];     // staged plane (+ Phi) has arrived in ring slot s
     unsigned long long ufull[NS];      // U* of ring slot s is complete
     unsigned long long pro;            // the three Phi planes of the prologue have arrived
+    unsigned long long dsync, esync;   // group barriers of the Lagrangian / the Eulerian warps
+    unsigned long long yrdy[FY], prdy[FY];   // row hand-offs of the Eulerian warps (see row_arrive)
     long long rowoff[FY];              // nx * (mapped y of footprint row)
     long long phirow[FY];              // pitch * (padded y of footprint row)
     int phi_len;                       // doubles of a Phi row that exist in the padded array
@@ -477,7 +475,7 @@ __device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b) {
 
 // Per-thread state of a Lagrangian thread: DROWS output cells (rows 2 + w + NDW q of the footprint, column lane).
 struct LagRows {
-    double Sz_prev[DROWS], wzp_prev[DROWS];
+    double Sz_prev[DROWS], wzp_prev[DROWS], pre[DROWS];
     double smax;
     int bad;
 };
@@ -496,8 +494,9 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
     constexpr unsigned UBYTES = PL * (16 * TR::NPAIR + (TR::LAST1 ? 8 : 0)), PBYTES = PL * 8;   // one staged plane: state, Phi
     const bool zout = g.bcz == GP_BC_OUTFLOW;
     const size_t nxny = (size_t)g.nx * g.ny;
+    const bool lane_out = lane >= 2 && lane <= FX - 3;
 #pragma unroll
-    for (int q = 0; q < DROWS; ++q) L.Sz_prev[q] = L.wzp_prev[q] = 0.0;
+    for (int q = 0; q < DROWS; ++q) L.Sz_prev[q] = L.wzp_prev[q] = L.pre[q] = 0.0;
     L.smax = 0.0; L.bad = 0;
     // prologue: Phi(z0-2 .. z0) for the first B and C, then the bundles of ring slots 0 and 1:
     // (U(z0), Phi(z0+1)) for E(z0-1) and (U(z0+1), Phi(z0+2)) for E(z0)
@@ -537,6 +536,12 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
             LagCoef lc;
             double out[NF];
             bool emit = false;
+            const int xv = b.x0 - 2 + lane, yv = b.y0 - 2 + ty;
+            const bool is_out = lane_out && xv < g.nx && yv < g.ny;
+            const size_t off = (size_t)xv + (size_t)g.nx * yv + (size_t)(j - 1) * nxny;
+            // one plane ahead: what this row's NEXT output cell needs from global memory besides the ring
+            const double pre = L.pre[q];
+            L.pre[q] = TR::early(a, off + nxny, is_out && do_wzp && j + 1 <= b.z1);
             const double Sz_new = sum9_wz(rs, t);             // 16 x
             if (bot_dup) L.Sz_prev[q] = Sz_new;
             if (do_wzp) {
@@ -545,7 +550,9 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
                     double wxm, wxp, wym, wyp;
                     face_vel_xy(tzj, t, wxm, wxp, wym, wyp);
                     lc = lag_coef(th * 0.015625, wxm, wxp, wym, wyp, L.wzp_prev[q], wzp);
-                    lagrange_lower<TR::NP2, TR::LAST1>(rm, t, lc, out);
+                    // centre first (always needed), then plane j-2, whose slot is handed over below
+                    lagrange_add<TR::NP2, TR::LAST1, true>(r0, t, lc.c0, out);
+                    if (lag_needed(lc.zm, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(rm, t, lc.zm, out);
                     emit = true;
                 }
                 L.wzp_prev[q] = wzp;
@@ -559,7 +566,7 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
                 double* dst = ring + ((it + 2) & 3) * TR::SLOT;
                 double* pdst = phir + ((it + 5) & (NPHI - 1)) * PL;
                 if (bulk) fence_proxy_async();
-                bar_sync(BAR_D, NTD);
+                group_sync(&T->dsync, it & 1);
                 if (bulk) {
                     if (dtid == 0) {
                         mbar_arrive_expect_tx(land, UBYTES + (more_phi ? PBYTES : 0u));
@@ -574,11 +581,12 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
             }
 
             if (emit) {
-                lagrange_rest<TR::NP2, TR::LAST1>(r0, rs, t, lc, out);
-                const int xv = b.x0 - 2 + lane, yv = b.y0 - 2 + ty;
-                const bool is_out = lane >= 2 && lane <= FX - 3 && xv < g.nx && yv < g.ny;
-                const size_t off = (size_t)xv + (size_t)g.nx * yv + (size_t)(j - 1) * nxny;
-                if (is_out) TR::emit(a, off, out, L.smax, L.bad);
+                if (lag_needed(lc.xm, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(r0, t - 1, lc.xm, out);
+                if (lag_needed(lc.xp, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(r0, t + 1, lc.xp, out);
+                if (lag_needed(lc.ym, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(r0, t - FX, lc.ym, out);
+                if (lag_needed(lc.yp, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(r0, t + FX, lc.yp, out);
+                if (lag_needed(lc.zp, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(rs, t, lc.zp, out);
+                if (is_out) TR::emit(a, off, out, pre, L.smax, L.bad);
             }
         }
     }
@@ -595,9 +603,12 @@ struct GasTraits {
     static constexpr bool LAST1 = true;
     static constexpr int SLOT = 2 * PP + PL;
     static constexpr int PLANES = 2 + 1 + 1 + NPHI + 2 + NS * 5 + 4;
-    __device__ static __forceinline__ void emit(const FusedArgs<NGAS>& a, size_t off, const double out[NGAS], double& smax, int& bad) {
-        double n_other = 0.0;
-        if (a.src_in) n_other = a.src_in[BSTR * off];
+    // density of the other component for the Poisson source, asked for one plane before it is used
+    __device__ static __forceinline__ double early(const FusedArgs<NGAS>& a, size_t off, bool is_out) {
+        return (a.src_in && is_out) ? a.src_in[BSTR * off] : 0.0;
+    }
+    __device__ static __forceinline__ void emit(const FusedArgs<NGAS>& a, size_t off, const double out[NGAS], double n_other, double& smax,
+                                                int& bad) {
 #pragma unroll
         for (int P = 0; P < NGASP / 2; ++P)
             *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
@@ -637,6 +648,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
     const double* ph0 = S.phi + ((it + 1) & (NPHI - 1)) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
+    if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
     // that the two solvers interleave.  Row FY-1 has no row above it; its faces are never used.
@@ -660,7 +672,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         c.amx = c.amx - th2 * (Pxh - Pxl) - trg;
         c.aE = c.aE - th4 * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
     }
-    bar_sync(BAR_E, NTE);
+    row_arrive(&T->yrdy[f.ty]);                                  // y fluxes of this row are written
+    if (f.ty > 0) mbar_wait(&T->yrdy[f.ty - 1], it & 1);       // ... and those of the row below
 
     // C: y-flux difference
     if (f.star_row) {
@@ -710,9 +723,10 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
     c.amx = mx_n; c.amy = my_n; c.amz = fma(th2, Pz, mz_n); c.aE = fma(th4, PVz, E_n);
     c.rho = rho_n; c.ir = ir_n; c.vx = vx_n; c.vy = vy_n; c.vz = vz_n; c.p = p_n;
-    bar_sync(BAR_E, NTE);
+    row_arrive(&T->prdy[f.ty]);                                  // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
+        group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
         if (f.fix) {
 #pragma unroll
             for (int P = 0; P < 2; ++P) {
@@ -726,9 +740,10 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
             const double2 v = lds2(S.tz + (it & 1) * PP + 2 * f.fix_src);
             sts2(S.tz + (it & 1) * PP + 2 * t, v.x, v.y);
         }
-        bar_sync(BAR_E, NTE);
+        group_sync(&T->esync, 0);
     }
-    if (threadIdx.x == 0) mbar_arrive(&T->ufull[it & 3]);
+    __syncwarp();
+    if (f.tx == 0) mbar_arrive(&T->ufull[it & 3]);   // this row's U*(j) is complete
 }
 
 __global__ void __launch_bounds__(NT, 1)
@@ -745,8 +760,11 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
     if (threadIdx.x == 0) {
         build_tab(T, g, a.phi, b, a.use_tma);
         const unsigned cnt = T->percell ? NTD : 1;
-        for (int s = 0; s < NS; ++s) { mbar_init(&T->landed[s], cnt); mbar_init(&T->ufull[s], 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(&T->landed[s], cnt); mbar_init(&T->ufull[s], NEW); }
         mbar_init(&T->pro, cnt);
+        mbar_init(&T->dsync, NDW);
+        mbar_init(&T->esync, NEW);
+        for (int r = 0; r < FY; ++r) { mbar_init(&T->yrdy[r], 1); mbar_init(&T->prdy[r], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -790,7 +808,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
             sts2(S.rp + 2 * t, c.rho, c.p); S.vx[t] = c.vx; S.vy[t] = c.vy;
         }
         mbar_wait(&T->pro, 0);
-        bar_sync(BAR_E, NTE);
+        group_sync(&T->esync, 0);
 
         int j = b.z0 - 1;
         for (; j <= b.z0 && j <= b.z1; ++j) gas_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
@@ -814,7 +832,8 @@ struct BmeTraits {
     static constexpr bool LAST1 = false;
     static constexpr int SLOT = 5 * PP;
     static constexpr int PLANES = 9 + NPHI + 9 + NS * 10 + 4;
-    __device__ static __forceinline__ void emit(const FusedArgs<NBME>& a, size_t off, const double out[NBME], double& smax, int& bad) {
+    __device__ static __forceinline__ double early(const FusedArgs<NBME>&, size_t, bool) { return 0.0; }
+    __device__ static __forceinline__ void emit(const FusedArgs<NBME>& a, size_t off, const double out[NBME], double, double& smax, int& bad) {
 #pragma unroll
         for (int P = 0; P < NBME / 2; ++P)
             *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
@@ -855,6 +874,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
     const double* ph0 = S.phi + ((it + 1) & (NPHI - 1)) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
+    if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
     // dependent chains interleave; rows 0 and FY-1 (halo rows whose results are never used) run them on
@@ -883,7 +903,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         gx = (ph0[te] - ph0[f.tx > 0 ? t - 1 : t]) * inv2h;
         gy = (ph0[tn] - ph0[f.ty > 0 ? t - FX : t]) * inv2h;
     }
-    bar_sync(BAR_E, NTE);
+    row_arrive(&T->yrdy[f.ty]);                                  // y fluxes of this row are written
+    if (f.ty > 0) mbar_wait(&T->yrdy[f.ty - 1], it & 1);       // ... and those of the row below
 
     // C: y-flux difference, then everything of U*(j) but the upper z face
     if (f.star_row) {
@@ -969,9 +990,10 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     for (int d = 0; d < 3; ++d) c.u[d] = u_n[d];
 #pragma unroll
     for (int q = 0; q < 6; ++q) c.Pi[q] = Pi_n[q];
-    bar_sync(BAR_E, NTE);
+    row_arrive(&T->prdy[f.ty]);                                  // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
+        group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
         if (f.fix) {
 #pragma unroll
             for (int P = 0; P < 5; ++P) {
@@ -982,9 +1004,10 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
             const double2 v = lds2(S.tz + (it & 1) * PP + 2 * f.fix_src);
             sts2(S.tz + (it & 1) * PP + 2 * t, v.x, v.y);
         }
-        bar_sync(BAR_E, NTE);
+        group_sync(&T->esync, 0);
     }
-    if (threadIdx.x == 0) mbar_arrive(&T->ufull[it & 3]);
+    __syncwarp();
+    if (f.tx == 0) mbar_arrive(&T->ufull[it & 3]);   // this row's U*(j) is complete
 }
 
 __global__ void __launch_bounds__(NT, 1)
@@ -1001,8 +1024,11 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
     if (threadIdx.x == 0) {
         build_tab(T, g, a.phi, b, a.use_tma);
         const unsigned cnt = T->percell ? NTD : 1;
-        for (int s = 0; s < NS; ++s) { mbar_init(&T->landed[s], cnt); mbar_init(&T->ufull[s], 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(&T->landed[s], cnt); mbar_init(&T->ufull[s], NEW); }
         mbar_init(&T->pro, cnt);
+        mbar_init(&T->dsync, NDW);
+        mbar_init(&T->esync, NEW);
+        for (int r = 0; r < FY; ++r) { mbar_init(&T->yrdy[r], 1); mbar_init(&T->prdy[r], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -1055,7 +1081,7 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
             sts2(S.py + 2 * t, c.Pi[3], c.Pi[4]); S.pxy[t] = c.Pi[1];
         }
         mbar_wait(&T->pro, 0);
-        bar_sync(BAR_E, NTE);
+        group_sync(&T->esync, 0);
 
         int j = b.z0 - 1;
         for (; j <= b.z0 && j <= b.z1; ++j) bme_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
