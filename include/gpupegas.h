@@ -125,6 +125,12 @@ int gp_timing_read(gp_ctx* ctx, int max_entries, int* n_entries, const char** na
  * own scratch; uses the default stream; synchronises. */
 int gp_math_selftest(int n, const double* x, double* rcp, double* rsqrt_out);
 
+/* ---- optional: self test of the fp64 issue rate of the device ----
+ * Runs a kernel of independent DFMA chains on every SM of the current device (default stream, synchronises) and
+ * returns the achieved fp64 thread-instructions per second (host pointer) and, if ms is not NULL, the best kernel
+ * time in milliseconds.  bench.py reports it beside the nominal fp64 peak of its ALU roofline. */
+int gp_fp64_rate_selftest(double* thread_inst_per_s, double* ms);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,7 +16,8 @@ BC_PERIODIC, BC_OUTFLOW = 0, 1
 OK, ERR_ARG, ERR_ALLOC, ERR_STATE, ERR_UNSUPPORTED = 0, 1, 2, 5, 6
 FIELDS = ["rho", "mx", "my", "mz", "E",
           "n", "nux", "nuy", "nuz", "Exx", "Exy", "Exz", "Eyy", "Eyz", "Ezz", "phi"]
-FIELD_ID = {name: i for i, name in enumerate(FIELDS)}
+OD_FIELDS = ["eps", "Pxx", "Pxy", "Pxz", "Pyy", "Pyz", "Pzz"]      # carried fields of the overdetermined system
+FIELD_ID = {name: i for i, name in enumerate(FIELDS + OD_FIELDS)}
 GAS_FIELDS = FIELDS[:5]
 STAR_FIELDS = FIELDS[5:15]
 
@@ -39,6 +40,12 @@ def lib():
             getattr(L, name).argtypes = [C.c_void_p, C.c_int, _dp]
         for name in ("orc_eulerian", "orc_lagrangian", "orc_lagrangian_only", "orc_step"):
             getattr(L, name).argtypes = [C.c_void_p, C.c_double]
+        for name in ("orc_od_eulerian", "orc_od_lagrangian", "orc_od_lagrangian_only"):
+            getattr(L, name).argtypes = [C.c_void_p, C.c_double]
+        L.orc_od_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.orc_od_enable.argtypes = [C.c_void_p]
+        L.orc_od_balance.argtypes = [C.c_void_p]
+        L.orc_kappa.argtypes = [C.c_void_p, _dp]
         L.orc_max_dt.argtypes = [C.c_void_p, C.c_double, _dp]
         L.orc_solve_poisson.argtypes = [C.c_void_p]
         L.orc_get_phi_padded.argtypes = [C.c_void_p, _dp]
@@ -142,6 +149,30 @@ class Oracle:
 
     def solve_poisson(self):
         _chk(lib().orc_solve_poisson(self._c), "solve_poisson")
+
+    # ---- overdetermined system (PAPER.md:41 4th equation, 65, 194-202) ----
+    def od_enable(self):
+        _chk(lib().orc_od_enable(self._c), "od_enable")
+
+    def od_field_names(self):
+        return (["eps"] if self.components & GAS else []) + (OD_FIELDS[1:] if self.components & STARS else [])
+
+    def od_eulerian(self, dt):
+        _chk(lib().orc_od_eulerian(self._c, dt), "od_eulerian")
+
+    def od_lagrangian_only(self, dt):
+        _chk(lib().orc_od_lagrangian_only(self._c, dt), "od_lagrangian_only")
+
+    def od_step(self, dt, balance=True):
+        _chk(lib().orc_od_step(self._c, dt, 1 if balance else 0), "od_step")
+
+    def od_balance(self):
+        _chk(lib().orc_od_balance(self._c), "od_balance")
+
+    def kappa(self):
+        out = np.zeros(2)
+        _chk(lib().orc_kappa(self._c, _p(out)), "kappa")
+        return float(out[0]), float(out[1])
 
 
 def gas_face(gamma, rhoL, vL, pL, rhoR, vR, pR):

@@ -57,6 +57,10 @@ struct orc_ctx {
     std::vector<double> phi;        // padded; face ghosts meaningful
     std::vector<double> kspec;      // isolated mode: real spectrum of the 1/r kernel on (2N)^3
     bool kspec_ready = false;
+    // overdetermined system (PAPER.md:41 4th equation; section "Overdetermined system" below)
+    bool od = false;
+    std::vector<double> eps, eps_s;         // rho*eps and its U*, padded
+    std::vector<double> Pi[6], Pi_s[6];     // Pi_ij (xx,xy,xz,yy,yz,zz) and their U*, padded
 
     inline std::size_t at(int i, int j, int k) const {   // i,j,k in [-1, n]
         return (std::size_t)(i + 1) + (std::size_t)px * ((std::size_t)(j + 1) + (std::size_t)py * (std::size_t)(k + 1));
@@ -488,6 +492,272 @@ int poisson_isolated(orc_ctx* c) {
     return ORC_OK;
 }
 
+// =============================================================================================
+// Overdetermined system and correctness check.
+//
+// GPUPEGAS carries the internal energy rho*eps beside the total energy rho*E (4th
+// equation) and the dispersion tensor Pi_ij beside n*E_ij, takes the pressure
+// p = (gamma-1) rho*eps and Pi_ij from the CARRIED fields, and measures how far the two
+// descriptions drift apart, kappa_gas and kappa_bme.  Everything below is
+// additional to the pinned scheme above, which it never calls into with different data:
+//   * eulerian_od: the stage of PAPER.md:72 with primitives from (rho, rho v, rho eps) and
+//     (n, n u, Pi); rho v, rho E, n u, n E_ij change by the same face values and formulas as in
+//     eulerian(); in addition (PAPER.md:41 without advection and cooling, PAPER.md:65 without advection)
+//       (rho eps)* = rho eps - tau (gamma-1) rho eps  sum_d (V_{d+1/2} - V_{d-1/2}) / h
+//       Pi_ij*     = Pi_ij   - tau sum_k [ Pi_jk (u*_i|_{k+1/2} - u*_i|_{k-1/2}) + Pi_ik (u*_j|_{k+1/2} - u*_j|_{k-1/2}) ] / h
+//     with V and u* the face values of 112 and 170-172 (the same the other equations use).
+//   * lagrangian_od: rho eps and Pi_ij are advected like every other field of their component.
+//   * kappa: PAPER.md:198-200 as Riemann sums, kappa_bme summed over the six independent components.
+//   * energy_balance: PAPER.md:202 only cites Vshivkov et al. (2011,2).  THIS PROCEDURE IS THE BUILD'S OWN
+//     DESIGN (reading G15): where the total-energy description is physical (rho E - rho v^2/2 > 0,
+//     resp. all three diagonal entries of n E_ij - n u_i u_j > 0) it wins and the carried field is reset from it, so
+//     total energy stays conserved; elsewhere (gas-vacuum borders, where that difference has gone non-positive) the
+//     carried, positive field wins: the gas velocity is rescaled in length, direction kept, so that rho v^2/2 =
+//     rho E - rho eps (set to zero, and rho E raised to rho eps, if even that is negative), and n E_ij is reset to
+//     Pi_ij + n u_i u_j.  Afterwards kappa_gas = kappa_bme = 0 and p, Pi_dd > 0 in every cell.
+// =============================================================================================
+void od_alloc(orc_ctx* c) {
+    if (c->od) return;
+    if (c->has_gas()) { c->eps.assign(c->npad, 0.0); c->eps_s.assign(c->npad, 0.0); }
+    if (c->has_stars())
+        for (int s = 0; s < 6; ++s) { c->Pi[s].assign(c->npad, 0.0); c->Pi_s[s].assign(c->npad, 0.0); }
+    c->od = true;
+}
+
+// rho*eps implied by the conserved fields (PAPER.md:41 last line): rho E - rho v^2/2, the kinetic energy written exactly
+// as S0 (gas_prim) writes it, so that (gamma-1) times this is bit for bit the pressure S0 recovers
+inline double gas_eint(const orc_ctx* c, std::size_t q) {
+    const double rho = c->U[ORC_RHO][q];
+    double v[3];
+    for (int i = 0; i < 3; ++i) v[i] = c->U[ORC_MX + i][q] / rho;
+    const double kin = 0.5 * rho * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    return c->U[ORC_E][q] - kin;
+}
+
+// carried fields := what the conserved fields imply (PAPER.md:41 last line); same expressions as S0
+void od_derive(orc_ctx* c) {
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                const std::size_t q = c->at(i, j, k);
+                if (c->has_gas()) c->eps[q] = gas_eint(c, q);
+                if (c->has_stars()) {
+                    const BmePrim w = bme_prim(c->U, q);
+                    for (int s = 0; s < 6; ++s) c->Pi[s][q] = w.Pi[s];
+                }
+            }
+}
+
+inline GasPrim gas_prim_od(const orc_ctx* c, std::size_t q) {
+    GasPrim w;
+    w.rho = c->U[ORC_RHO][q];
+    for (int i = 0; i < 3; ++i) w.v[i] = c->U[ORC_MX + i][q] / w.rho;
+    w.p = (c->gamma - 1.0) * c->eps[q];                     // pressure from the carried internal energy
+    return w;
+}
+
+inline BmePrim bme_prim_od(const orc_ctx* c, std::size_t q) {
+    BmePrim w;
+    w.n = c->U[ORC_N][q];
+    for (int i = 0; i < 3; ++i) w.u[i] = c->U[ORC_NUX + i][q] / w.n;
+    for (int s = 0; s < 6; ++s) w.Pi[s] = c->Pi[s][q];      // dispersion tensor as carried
+    return w;
+}
+
+void eulerian_od(orc_ctx* c, double tau) {
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const double h = c->h;
+    if (c->has_gas()) {
+        for (int f = 0; f < NGAS; ++f) ghost_fill(c, c->U[f], c->bc);
+        ghost_fill(c, c->eps, c->bc);
+    }
+    if (c->has_stars()) {
+        for (int f = NGAS; f < NHYD; ++f) ghost_fill(c, c->U[f], c->bc);
+        for (int s = 0; s < 6; ++s) ghost_fill(c, c->Pi[s], c->bc);
+    }
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const std::size_t q = c->at(i, j, k);
+                double g[3];
+                for (int d = 0; d < 3; ++d)
+                    g[d] = (c->phi[q + c->stride(d)] - c->phi[q - c->stride(d)]) / (2.0 * h);
+
+                if (c->has_gas()) {
+                    const GasPrim w0 = gas_prim_od(c, q);
+                    double dP[3], dPV = 0.0, divV = 0.0;
+                    for (int d = 0; d < 3; ++d) {
+                        const GasPrim wm = gas_prim_od(c, q - c->stride(d));
+                        const GasPrim wp = gas_prim_od(c, q + c->stride(d));
+                        double Vm, Pm, Vp, Pp;
+                        gas_face(c->gamma, wm.rho, wm.v[d], wm.p, w0.rho, w0.v[d], w0.p, Vm, Pm);
+                        gas_face(c->gamma, w0.rho, w0.v[d], w0.p, wp.rho, wp.v[d], wp.p, Vp, Pp);
+                        dP[d] = Pp - Pm;
+                        dPV += Pp * Vp - Pm * Vm;
+                        divV += Vp - Vm;
+                    }
+                    c->Us[ORC_RHO][q] = w0.rho;
+                    double work = 0.0;
+                    for (int d = 0; d < 3; ++d) {
+                        const double m = c->U[ORC_MX + d][q];
+                        c->Us[ORC_MX + d][q] = m - tau / h * dP[d] - tau * w0.rho * g[d];
+                        work += (m - 0.5 * tau * w0.rho * g[d]) * g[d];
+                    }
+                    c->Us[ORC_E][q] = c->U[ORC_E][q] - tau / h * dPV - tau * work;
+                    // PAPER.md:41, 4th equation, without advection and cooling
+                    c->eps_s[q] = c->eps[q] - tau / h * (c->gamma - 1.0) * c->eps[q] * divV;
+                }
+
+                if (c->has_stars()) {
+                    const BmePrim w0 = bme_prim_od(c, q);
+                    double dnu[3] = {0, 0, 0}, dE[6] = {0, 0, 0, 0, 0, 0};
+                    double du[3][3];                         // du[i][k] = u*_i|_{k+1/2} - u*_i|_{k-1/2}
+                    for (int d = 0; d < 3; ++d) {
+                        const BmePrim wm = bme_prim_od(c, q - c->stride(d));
+                        const BmePrim wp = bme_prim_od(c, q + c->stride(d));
+                        double um[3], Pm[3], up[3], Pp[3];
+                        bme_face(d, wm.n, wm.u, wm.Pi, w0.n, w0.u, w0.Pi, um, Pm);
+                        bme_face(d, w0.n, w0.u, w0.Pi, wp.n, wp.u, wp.Pi, up, Pp);
+                        for (int a = 0; a < 3; ++a) dnu[a] += Pp[a] - Pm[a];
+                        for (int a = 0; a < 3; ++a)
+                            for (int b = a; b < 3; ++b)
+                                dE[sym(a, b)] += (Pp[b] * up[a] + Pp[a] * up[b]) - (Pm[b] * um[a] + Pm[a] * um[b]);
+                        for (int a = 0; a < 3; ++a) du[a][d] = up[a] - um[a];
+                    }
+                    c->Us[ORC_N][q] = w0.n;
+                    for (int a = 0; a < 3; ++a)
+                        c->Us[ORC_NUX + a][q] = c->U[ORC_NUX + a][q] - tau / h * dnu[a] - tau * w0.n * g[a];
+                    for (int a = 0; a < 3; ++a)
+                        for (int b = a; b < 3; ++b) {
+                            const double src = (w0.u[a] - 0.5 * tau * g[a]) * g[b] + (w0.u[b] - 0.5 * tau * g[b]) * g[a];
+                            c->Us[ORC_EXX + sym(a, b)][q] =
+                                c->U[ORC_EXX + sym(a, b)][q] - tau / h * dE[sym(a, b)] - tau * w0.n * src;
+                            // PAPER.md:65 without advection: -Pi_jk du_i/dx_k - Pi_ik du_j/dx_k  (i = a, j = b)
+                            double rhs = 0.0;
+                            for (int kk = 0; kk < 3; ++kk)
+                                rhs += w0.Pi[sym(b, kk)] * du[a][kk] + w0.Pi[sym(a, kk)] * du[b][kk];
+                            c->Pi_s[sym(a, b)][q] = w0.Pi[sym(a, b)] - tau / h * rhs;
+                        }
+                }
+            }
+}
+
+// PAPER.md:124 for a list of fields that move with the velocity w* = Us[mom0 + d] / Us[dens] (same loop body as
+// lagrangian_component; the extra fields of the overdetermined system ride along)
+void lagrangian_fields(orc_ctx* c, double tau, std::vector<std::vector<double>*> star, std::vector<std::vector<double>*> out,
+                       int dens, int mom0) {
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const double h = c->h;
+    for (auto* a : star) ghost_fill(c, *a, c->bc);
+    std::vector<double> w[3];
+    for (int d = 0; d < 3; ++d) {
+        w[d].resize(c->npad);
+        for (std::size_t q = 0; q < c->npad; ++q) w[d][q] = c->Us[mom0 + d][q] / c->Us[dens][q];
+    }
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const std::size_t q = c->at(i, j, k);
+                double wm[3], wp[3];
+                for (int d = 0; d < 3; ++d) {
+                    wm[d] = face_velocity(c, w[d], q - c->stride(d), d);
+                    wp[d] = face_velocity(c, w[d], q, d);
+                }
+                for (std::size_t f = 0; f < star.size(); ++f) {
+                    const std::vector<double>& fs = *star[f];
+                    double div = 0.0;
+                    for (int d = 0; d < 3; ++d) {
+                        const std::size_t sd = c->stride(d);
+                        const double Fp = wp[d] * (wp[d] >= 0.0 ? fs[q] : fs[q + sd]);
+                        const double Fm = wm[d] * (wm[d] >= 0.0 ? fs[q - sd] : fs[q]);
+                        div += Fp - Fm;
+                    }
+                    (*out[f])[q] = fs[q] - tau / h * div;
+                }
+            }
+}
+
+void lagrangian_od(orc_ctx* c, double tau) {
+    if (c->has_gas()) {
+        std::vector<std::vector<double>*> s, o;
+        for (int f = 0; f < NGAS; ++f) { s.push_back(&c->Us[f]); o.push_back(&c->U[f]); }
+        s.push_back(&c->eps_s); o.push_back(&c->eps);
+        lagrangian_fields(c, tau, s, o, ORC_RHO, ORC_MX);
+    }
+    if (c->has_stars()) {
+        std::vector<std::vector<double>*> s, o;
+        for (int f = NGAS; f < NHYD; ++f) { s.push_back(&c->Us[f]); o.push_back(&c->U[f]); }
+        for (int q = 0; q < 6; ++q) { s.push_back(&c->Pi_s[q]); o.push_back(&c->Pi[q]); }
+        lagrangian_fields(c, tau, s, o, ORC_N, ORC_NUX);
+    }
+}
+
+// PAPER.md:198-200 as Riemann sums over the cells (volume h^3)
+void kappa(const orc_ctx* c, double out[2]) {
+    double kg = 0.0, kb = 0.0;
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                const std::size_t q = c->at(i, j, k);
+                if (c->has_gas()) {
+                    const double rho = c->U[ORC_RHO][q];
+                    double v2 = 0.0;
+                    for (int d = 0; d < 3; ++d) { const double v = c->U[ORC_MX + d][q] / rho; v2 += v * v; }
+                    kg += std::fabs(c->U[ORC_E][q] - c->eps[q] - 0.5 * rho * v2);
+                }
+                if (c->has_stars()) {
+                    const double n = c->U[ORC_N][q];
+                    double u[3];
+                    for (int d = 0; d < 3; ++d) u[d] = c->U[ORC_NUX + d][q] / n;
+                    for (int a = 0; a < 3; ++a)
+                        for (int b = a; b < 3; ++b)
+                            kb += std::fabs(c->U[ORC_EXX + sym(a, b)][q] - c->Pi[sym(a, b)][q] - n * u[a] * u[b]);
+                }
+            }
+    const double h3 = c->h * c->h * c->h;
+    out[0] = kg * h3;
+    out[1] = kb * h3;
+}
+
+// The build's own reading of "energy balance procedure", see the section header (G15).
+void energy_balance(orc_ctx* c) {
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                const std::size_t q = c->at(i, j, k);
+                if (c->has_gas()) {
+                    const GasPrim w = gas_prim(c, c->U, q);
+                    const double e_tot = gas_eint(c, q);                // rho eps as the total energy implies it
+                    if (e_tot > 0.0) {
+                        c->eps[q] = e_tot;                                  // total energy wins
+                    } else {
+                        const double rho = w.rho;
+                        const double kin_new = c->U[ORC_E][q] - c->eps[q];  // what rho v^2/2 has to be
+                        const double kin_old = 0.5 * rho * (w.v[0] * w.v[0] + w.v[1] * w.v[1] + w.v[2] * w.v[2]);
+                        if (kin_new > 0.0 && kin_old > 0.0) {
+                            const double s = std::sqrt(kin_new / kin_old);  // length of v rescaled, direction kept
+                            for (int d = 0; d < 3; ++d) c->U[ORC_MX + d][q] *= s;
+                        } else {
+                            for (int d = 0; d < 3; ++d) c->U[ORC_MX + d][q] = 0.0;
+                            c->U[ORC_E][q] = c->eps[q];
+                        }
+                    }
+                }
+                if (c->has_stars()) {
+                    const BmePrim w = bme_prim(c->U, q);
+                    if (w.Pi[0] > 0.0 && w.Pi[3] > 0.0 && w.Pi[5] > 0.0) {
+                        for (int s = 0; s < 6; ++s) c->Pi[s][q] = w.Pi[s];
+                    } else {
+                        for (int a = 0; a < 3; ++a)
+                            for (int b = a; b < 3; ++b)
+                                c->U[ORC_EXX + sym(a, b)][q] = c->Pi[sym(a, b)][q] + w.n * w.u[a] * w.u[b];
+                    }
+                }
+            }
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -532,6 +802,14 @@ int orc_get_threads(void) {
 #endif
 }
 
+// the carried fields of the overdetermined system, or null
+static std::vector<double>* od_field(orc_ctx* c, int f, bool star) {
+    if (!c->od) return nullptr;
+    if (f == ORC_EPS && c->has_gas()) return star ? &c->eps_s : &c->eps;
+    if (f >= ORC_PXX && f <= ORC_PZZ && c->has_stars()) return star ? &c->Pi_s[f - ORC_PXX] : &c->Pi[f - ORC_PXX];
+    return nullptr;
+}
+
 static bool field_on(const orc_ctx* c, int f) {
     if (f < 0 || f >= ORC_NFIELDS) return false;
     if (f == ORC_PHI) return true;
@@ -539,8 +817,10 @@ static bool field_on(const orc_ctx* c, int f) {
 }
 
 int orc_set_field(orc_ctx* c, int field, const double* src) {
-    if (!c || !src || !field_on(c, field)) return ORC_ERR_ARG;
-    std::vector<double>& a = field == ORC_PHI ? c->phi : c->U[field];
+    if (!c || !src) return ORC_ERR_ARG;
+    std::vector<double>* extra = od_field(c, field, false);
+    if (!extra && !field_on(c, field)) return ORC_ERR_ARG;
+    std::vector<double>& a = extra ? *extra : (field == ORC_PHI ? c->phi : c->U[field]);
     for (int k = 0; k < c->nz; ++k)
         for (int j = 0; j < c->ny; ++j)
             for (int i = 0; i < c->nx; ++i)
@@ -558,13 +838,68 @@ static int get_from(orc_ctx* c, const std::vector<double>& a, double* dst) {
 }
 
 int orc_get_field(orc_ctx* c, int field, double* dst) {
-    if (!c || !dst || !field_on(c, field)) return ORC_ERR_ARG;
+    if (!c || !dst) return ORC_ERR_ARG;
+    if (std::vector<double>* extra = od_field(c, field, false)) return get_from(c, *extra, dst);
+    if (!field_on(c, field)) return ORC_ERR_ARG;
     return get_from(c, field == ORC_PHI ? c->phi : c->U[field], dst);
 }
 
 int orc_get_star_field(orc_ctx* c, int field, double* dst) {
-    if (!c || !dst || !field_on(c, field) || field == ORC_PHI) return ORC_ERR_ARG;
+    if (!c || !dst) return ORC_ERR_ARG;
+    if (std::vector<double>* extra = od_field(c, field, true)) return get_from(c, *extra, dst);
+    if (!field_on(c, field) || field == ORC_PHI) return ORC_ERR_ARG;
     return get_from(c, c->Us[field], dst);
+}
+
+/* ---- overdetermined system ---- */
+int orc_od_enable(orc_ctx* c) {
+    if (!c) return ORC_ERR_ARG;
+    try { od_alloc(c); } catch (...) { return ORC_ERR_ALLOC; }
+    od_derive(c);
+    return ORC_OK;
+}
+
+int orc_od_eulerian(orc_ctx* c, double dt) {
+    if (!c || !c->od || !(dt >= 0.0)) return ORC_ERR_ARG;
+    eulerian_od(c, dt);
+    return ORC_OK;
+}
+
+int orc_od_lagrangian(orc_ctx* c, double dt) {
+    if (!c || !c->od || !(dt >= 0.0)) return ORC_ERR_ARG;
+    lagrangian_od(c, dt);
+    return ORC_OK;
+}
+
+int orc_od_lagrangian_only(orc_ctx* c, double dt) {
+    if (!c || !c->od || !(dt >= 0.0)) return ORC_ERR_ARG;
+    for (int f = 0; f < NHYD; ++f)
+        if (field_on(c, f)) c->Us[f] = c->U[f];
+    if (c->has_gas()) c->eps_s = c->eps;
+    if (c->has_stars())
+        for (int s = 0; s < 6; ++s) c->Pi_s[s] = c->Pi[s];
+    lagrangian_od(c, dt);
+    return ORC_OK;
+}
+
+int orc_od_step(orc_ctx* c, double dt, int balance) {
+    if (!c || !c->od || !(dt > 0.0)) return ORC_ERR_ARG;
+    eulerian_od(c, dt);
+    lagrangian_od(c, dt);
+    if (balance) energy_balance(c);
+    return ORC_OK;
+}
+
+int orc_od_balance(orc_ctx* c) {
+    if (!c || !c->od) return ORC_ERR_ARG;
+    energy_balance(c);
+    return ORC_OK;
+}
+
+int orc_kappa(orc_ctx* c, double* out) {
+    if (!c || !c->od || !out) return ORC_ERR_ARG;
+    kappa(c, out);
+    return ORC_OK;
 }
 
 int orc_get_phi_padded(orc_ctx* c, double* dst) {

@@ -28,7 +28,9 @@ enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1 };
  * n, n*u (3), nE_xx, nE_xy, nE_xz, nE_yy, nE_yz, nE_zz; potential Phi+Phi0. */
 enum { ORC_RHO = 0, ORC_MX, ORC_MY, ORC_MZ, ORC_E,
        ORC_N, ORC_NUX, ORC_NUY, ORC_NUZ, ORC_EXX, ORC_EXY, ORC_EXZ, ORC_EYY, ORC_EYZ, ORC_EZZ,
-       ORC_PHI, ORC_NFIELDS };
+       ORC_PHI, ORC_NFIELDS,
+       /* carried fields of the overdetermined system (orc_od_*): rho*eps, Pi_ij */
+       ORC_EPS = ORC_NFIELDS, ORC_PXX, ORC_PXY, ORC_PXZ, ORC_PYY, ORC_PYZ, ORC_PZZ };
 
 orc_ctx* orc_create(int nx, int ny, int nz, double h, int components, int poisson, double G,
                     double gamma, int bcx, int bcy, int bcz);
@@ -48,6 +50,20 @@ int orc_max_dt(orc_ctx*, double cfl, double* dt);
 int orc_solve_poisson(orc_ctx*);
 /* Phi including its one-cell ghost ring, (nx+2)(ny+2)(nz+2) doubles, x fastest. */
 int orc_get_phi_padded(orc_ctx*, double* dst);
+
+/* ---- overdetermined system and correctness check ----
+ * orc_od_enable allocates rho*eps and Pi_ij and derives them from the current conserved state; afterwards
+ * orc_set_field / orc_get_field / orc_get_star_field accept ORC_EPS and ORC_PXX..ORC_PZZ.  The orc_od_* stages take
+ * the pressure and the dispersion tensor from the CARRIED fields and update them by their own equations.
+ * orc_kappa: out[0] = kappa_gas, out[1] = kappa_bme.  orc_od_balance is the build's own reading
+ * of the "energy balance procedure" the paper only cites (G15). */
+int orc_od_enable(orc_ctx*);
+int orc_od_eulerian(orc_ctx*, double dt);
+int orc_od_lagrangian(orc_ctx*, double dt);
+int orc_od_lagrangian_only(orc_ctx*, double dt);
+int orc_od_step(orc_ctx*, double dt, int balance);
+int orc_od_balance(orc_ctx*);
+int orc_kappa(orc_ctx*, double* out);
 
 /* ---- stateless pieces, exported so tests can pin them one by one ---- */
 /* PAPER.md:112,114 */

@@ -22,7 +22,8 @@ GAS_FIELDS, STAR_FIELDS = FIELDS[:5], FIELDS[5:15]
 # the symbols include/gpupegas.h declares
 EXPORTS = ["gp_create", "gp_destroy", "gp_set_state", "gp_get_state", "gp_solve_poisson", "gp_max_dt",
            "gp_step", "gp_last_error", "gp_set_stream", "gp_storage_bytes", "gp_bind_storage",
-           "gp_synchronize", "gp_launch_counts", "gp_timing_enable", "gp_timing_read", "gp_math_selftest"]
+           "gp_synchronize", "gp_launch_counts", "gp_timing_enable", "gp_timing_read", "gp_math_selftest",
+           "gp_fp64_rate_selftest"]
 
 
 class gp_grid(C.Structure):
@@ -71,6 +72,7 @@ def lib():
         L.gp_timing_enable.argtypes = [vp, C.c_int]
         L.gp_timing_read.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_char_p), dp, C.POINTER(C.c_longlong)]
         L.gp_math_selftest.argtypes = [C.c_int, vp, vp, vp]
+        L.gp_fp64_rate_selftest.argtypes = [dp, dp]
         _lib = L
     return _lib
 
@@ -82,6 +84,13 @@ def math_selftest(x):
     r, s = np.empty_like(x), np.empty_like(x)
     _chk(lib().gp_math_selftest(x.size, x.ctypes.data, r.ctypes.data, s.ctypes.data), "gp_math_selftest")
     return r, s
+
+
+def fp64_rate_selftest():
+    """(fp64 thread-instructions per second, kernel ms) of the DFMA self test on the current device."""
+    rate, ms = C.c_double(0.0), C.c_double(0.0)
+    _chk(lib().gp_fp64_rate_selftest(C.byref(rate), C.byref(ms)), "gp_fp64_rate_selftest")
+    return rate.value, ms.value
 
 
 def _chk(code, what):

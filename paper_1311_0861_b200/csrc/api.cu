@@ -414,6 +414,11 @@ int gp_step(gp_ctx* c, double dt) {
     return GP_OK;
 }
 
+int gp_fp64_rate_selftest(double* thread_inst_per_s, double* ms) {
+    if (!thread_inst_per_s) { set_error("gp_fp64_rate_selftest: NULL argument"); return GP_ERR_ARG; }
+    return fp64_rate_selftest(thread_inst_per_s, ms);
+}
+
 int gp_math_selftest(int n, const double* x, double* rcp, double* rsqrt_out) {
     if (n < 1 || !x || !rcp || !rsqrt_out) { set_error("gp_math_selftest: bad argument"); return GP_ERR_ARG; }
     return math_selftest(n, x, rcp, rsqrt_out);

@@ -651,14 +651,14 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
-    // that the two solvers interleave.  Row FY-1 has no row above it; its faces are never used.
+    // that the two solvers interleave
     double Pyh = 0.0, PVyh = 0.0, gy = 0.0;
-    if (f.ty <= FY - 2) {
+    if (f.star_row) {
         const int tr = f.tx < FX - 1 ? t + 1 : t;
         const double2 ry = lds2(S.rp + 2 * (t + FX)), rx = lds2(S.rp + 2 * tr);
         const double vyr = S.vy[t + FX], vxr = S.vx[tr];
         const double phe = ph0[tr], phn = ph0[t + FX];
-        const double phw = ph0[f.tx > 0 ? t - 1 : t], phs = ph0[f.ty > 0 ? t - FX : t];
+        const double phw = ph0[f.tx > 0 ? t - 1 : t], phs = ph0[t - FX];
         double Pxh, PVxh;
         gas_face(gamma, c.rho, c.vy, c.p, ry.x, vyr, ry.y, Pyh, PVyh);
         gas_face(gamma, c.rho, c.vx, c.p, rx.x, vxr, rx.y, Pxh, PVxh);
@@ -671,6 +671,11 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         const double mx = c.rho * c.vx;
         c.amx = c.amx - th2 * (Pxh - Pxl) - trg;
         c.aE = c.aE - th4 * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
+    } else if (f.ty == 0) {
+        // the lowest halo row only supplies the y face between itself and row 1; the top halo row supplies nothing
+        const double2 ry = lds2(S.rp + 2 * (t + FX));
+        gas_face(gamma, c.rho, c.vy, c.p, ry.x, S.vy[t + FX], ry.y, Pyh, PVyh);
+        sts2(S.fy + 2 * t, Pyh, PVyh);
     }
     row_arrive(&T->yrdy[f.ty]);                                  // y fluxes of this row are written
     if (f.ty > 0) mbar_wait(&T->yrdy[f.ty - 1], it & 1);       // ... and those of the row below
@@ -877,12 +882,11 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
-    // dependent chains interleave; rows 0 and FY-1 (halo rows whose results are never used) run them on
-    // whatever they read
-    double Py[3], EFy[6];
-    double gx, gy;
-    {
-        const int tn = f.ty < FY - 1 ? t + FX : t, te = f.tx < FX - 1 ? t + 1 : t;
+    // dependent chains interleave
+    double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double gx = 0.0, gy = 0.0;
+    if (f.star_row) {
+        const int tn = t + FX, te = f.tx < FX - 1 ? t + 1 : t;
         const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
         const double2 x0 = lds2(S.nu + 2 * te), x1 = lds2(S.uu + 2 * te), x2 = lds2(S.px + 2 * te);
         const double pxy_n = S.pxy[tn], pxy_e = S.pxy[te];
@@ -901,7 +905,19 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
 #pragma unroll
         for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th4 * (EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1));
         gx = (ph0[te] - ph0[f.tx > 0 ? t - 1 : t]) * inv2h;
-        gy = (ph0[tn] - ph0[f.ty > 0 ? t - FX : t]) * inv2h;
+        gy = (ph0[tn] - ph0[t - FX]) * inv2h;
+    } else if (f.ty == 0) {
+        // the lowest halo row only supplies the y face between itself and row 1; the top halo row supplies nothing
+        const int tn = t + FX;
+        const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
+        const double ury[3] = {y0.y, y1.x, y1.y};
+        const double Ply[3] = {c.Pi[1], c.Pi[3], c.Pi[4]};
+        const double Pry[3] = {S.pxy[tn], y2.x, y2.y};
+        bme_face<1>(c.n, c.u, Ply, y0.x, ury, Pry, Py, EFy);
+        double* fy = S.fy;
+        sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
+        sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
+        fy[4 * PP + t] = EFy[5];
     }
     row_arrive(&T->yrdy[f.ty]);                                  // y fluxes of this row are written
     if (f.ty > 0) mbar_wait(&T->yrdy[f.ty - 1], it & 1);       // ... and those of the row below

@@ -138,6 +138,9 @@ int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src
 int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt);
 int math_selftest(int n, const double* x, double* rcp, double* rsq);
 
+// selftest.cu
+int fp64_rate_selftest(double* thread_inst_per_s, double* ms_out);
+
 // poisson.cu
 int poisson_setup(gp_ctx* c);
 void poisson_teardown(gp_ctx* c);

@@ -390,3 +390,13 @@ def test_isolated_poisson_ghost_faces_drive_the_same_step_as_the_oracle(pkg, orc
     ref.step(dt)
     for g in GROUPS_GAS:
         assert err_max(sim, ref, g) <= TOL_1STEP, g
+
+
+def test_fp64_issue_rate_self_test_backs_the_alu_peak(pkg):
+    """bench.py's roofline_alu takes 148 SMs x 64 fp64 lanes x the SM clock as the peak; the DFMA self test of the
+    library (csrc/selftest.cu) must reach most of it and cannot exceed it."""
+    import torch
+    rate, ms = pkg.fp64_rate_selftest()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    nominal = sms * 64 * 1.965e9
+    assert 0.75 * nominal <= rate <= 1.02 * nominal, (rate, nominal, ms)
