@@ -77,6 +77,12 @@ __device__ __forceinline__ int zidx(int t, int b, int m) {
     return (u / Q) * L + (u % Q) + m * Q;
 }
 
+// Shared-memory slot of element idx of a column.  The closing stages address elements 8 apart from consecutive threads
+// (Q = 1: idx = 8 t + m), which would put the eight t values of a warp on the same banks (C * 16 B * 8 = a multiple of
+// 128 B): XOR the low three bits with the next three.  Within an aligned group of eight elements this is a permutation,
+// so the stages whose threads walk consecutive elements stay conflict-free.
+__device__ __forceinline__ int zslot(int idx) { return idx ^ ((idx >> 3) & 7); }
+
 template <int P, int C, int s>
 struct ZExchange {
     // registers (stage s layout) -> shared -> registers (stage s2 layout)
@@ -87,12 +93,12 @@ struct ZExchange {
 #pragma unroll
         for (int b = 0; b < 8 / R; ++b)
 #pragma unroll
-            for (int m = 0; m < R; ++m) sm[zidx<P, R, L>(t, b, m) * C + col] = v[b * R + m];
+            for (int m = 0; m < R; ++m) sm[zslot(zidx<P, R, L>(t, b, m)) * C + col] = v[b * R + m];
         __syncthreads();
 #pragma unroll
         for (int b = 0; b < 8 / R2; ++b)
 #pragma unroll
-            for (int m = 0; m < R2; ++m) v[b * R2 + m] = sm[zidx<P, R2, L2>(t, b, m) * C + col];
+            for (int m = 0; m < R2; ++m) v[b * R2 + m] = sm[zslot(zidx<P, R2, L2>(t, b, m)) * C + col];
     }
 };
 

@@ -9,6 +9,7 @@
 #define GP_BME_REG_E 104
 #define GP_BME_REG_D 80
 #endif
+#define GP_NS 4
 #define GP_FY GP_BME_FY
 #define GP_NDW GP_BME_NDW
 #define GP_REG_E GP_BME_REG_E

@@ -8,6 +8,10 @@
 #define GP_GAS_REG_E 72
 #define GP_GAS_REG_D 64
 #endif
+#ifndef GP_GAS_NS
+#define GP_GAS_NS 6
+#endif
+#define GP_NS GP_GAS_NS
 #define GP_FY GP_GAS_FY
 #define GP_NDW GP_GAS_NDW
 #define GP_REG_E GP_GAS_REG_E

@@ -53,8 +53,17 @@ constexpr int NEW = FY;                   // Eulerian warps, one per footprint r
 constexpr int NDW = GP_NDW;               // Lagrangian / producer warps
 constexpr int NTE = NEW * 32, NTD = NDW * 32, NT = NTE + NTD;
 constexpr int DROWS = TYO / NDW;          // output rows per Lagrangian warp
-constexpr int NS = 4;                     // slots of the U* ring
-constexpr int NPHI = 8;                   // slots of the Phi ring
+#ifndef GP_NS
+#define GP_NS 4
+#endif
+constexpr int NS = GP_NS;                 // slots of the U* ring: planes j-2, j-1, j of the Lagrangian warps and NS - 3 ahead
+constexpr int NPHI = NS + 2;              // slots of the Phi ring
+constexpr int NTZ = NS - 2;               // buffers of the z-averaged face-velocity plane
+static_assert(NS >= 4, "the ring holds three planes for the Lagrangian stage and at least one ahead");
+// ring slot / mbarrier phase parity of plane index it (>= 0, counted from the first plane of the block)
+__host__ __device__ constexpr int rslot(int it) { return it % NS; }
+__host__ __device__ constexpr unsigned rpar(int it) { return (unsigned)(it / NS) & 1u; }
+__host__ __device__ constexpr int pslot(int k) { return k % NPHI; }
 static_assert(TYO % NDW == 0, "output rows must divide among the Lagrangian warps");
 
 // register budgets after the split (0: leave the launch allocation alone)
@@ -495,50 +504,53 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
     const bool zout = g.bcz == GP_BC_OUTFLOW;
     const size_t nxny = (size_t)g.nx * g.ny;
     const bool lane_out = lane >= 2 && lane <= FX - 3;
+    bool row_out[DROWS];         // this thread's cell of row q is an output cell of the grid, at row_off[q] in its plane
+    size_t row_off[DROWS];
 #pragma unroll
-    for (int q = 0; q < DROWS; ++q) L.Sz_prev[q] = L.wzp_prev[q] = L.pre[q] = 0.0;
-    L.smax = 0.0; L.bad = 0;
-    // prologue: Phi(z0-2 .. z0) for the first B and C, then the bundles of ring slots 0 and 1:
-    // (U(z0), Phi(z0+1)) for E(z0-1) and (U(z0+1), Phi(z0+2)) for E(z0)
-    const bool phi2 = b.z0 + 1 <= b.z1;       // C(z0+1) exists and needs Phi(z0+2)
-    if (bulk && dtid == 0) {
-        mbar_arrive_expect_tx(&T->pro, 3 * PBYTES);
-        mbar_arrive_expect_tx(&T->landed[0], UBYTES + PBYTES);
-        mbar_arrive_expect_tx(&T->landed[1], UBYTES + (phi2 ? PBYTES : 0u));
+    for (int q = 0; q < DROWS; ++q) {
+        const int xv = b.x0 - 2 + lane, yv = b.y0 + dw + NDW * q;
+        row_out[q] = lane_out && xv < g.nx && yv < g.ny;
+        row_off[q] = (size_t)xv + (size_t)g.nx * yv;
+        L.Sz_prev[q] = L.wzp_prev[q] = L.pre[q] = 0.0;
     }
+    L.smax = 0.0; L.bad = 0;
+    // prologue: Phi(z0-2 .. z0) for the first B and C, then the bundles (U(k+1), Phi(k+2)) of the first NS - 2 planes
+    // k = z0-1 ... into ring slots 0 ...; E(k) consumes bundle k
+    if (bulk && dtid == 0) mbar_arrive_expect_tx(&T->pro, 3 * PBYTES);
     __syncwarp();
     for (int k = 0; k < 3; ++k) stage_phi(a, T, b, phir + k * PL, b.z0 - 2 + k, &T->pro, dtid);
     if (!bulk) mbar_arrive_on_cp_async(&T->pro);
-    stage_state<TR::NPAIR, TR::LAST1>(a, T, b, ring, b.z0, &T->landed[0], dtid);
-    stage_phi(a, T, b, phir + 3 * PL, b.z0 + 1, &T->landed[0], dtid);
-    if (!bulk) mbar_arrive_on_cp_async(&T->landed[0]);
-    stage_state<TR::NPAIR, TR::LAST1>(a, T, b, ring + TR::SLOT, b.z0 + 1, &T->landed[1], dtid);
-    if (phi2) stage_phi(a, T, b, phir + 4 * PL, b.z0 + 2, &T->landed[1], dtid);
-    if (!bulk) mbar_arrive_on_cp_async(&T->landed[1]);
+    for (int i = 0; i < NS - 2 && j0 + i <= b.z1; ++i) {
+        const bool with_phi = j0 + i + 1 <= b.z1;        // C(k+1) exists and needs Phi(k+2)
+        if (bulk && dtid == 0) mbar_arrive_expect_tx(&T->landed[i], UBYTES + (with_phi ? PBYTES : 0u));
+        __syncwarp();
+        stage_state<TR::NPAIR, TR::LAST1>(a, T, b, ring + i * TR::SLOT, j0 + i + 1, &T->landed[i], dtid);
+        if (with_phi) stage_phi(a, T, b, phir + pslot(i + 3) * PL, j0 + i + 2, &T->landed[i], dtid);
+        if (!bulk) mbar_arrive_on_cp_async(&T->landed[i]);
+    }
 
     for (int j = j0; j <= b.z1; ++j) {
         const int it = j - j0;
         const bool bot_dup = zout && j == 0;
         const bool do_out = j - 1 >= b.z0;
         const bool do_wzp = j >= b.z0;
-        const double* rs = ring + (it & 3) * TR::SLOT;
-        const double* r0 = ring + ((it + 3) & 3) * TR::SLOT;
-        const double* rm = ring + ((it + 2) & 3) * TR::SLOT;
-        const double* tzj = tz + (it & 1) * PP;
-        mbar_wait(&T->ufull[it & 3], (it >> 2) & 1);      // U*(j) complete
+        const double* rs = ring + rslot(it) * TR::SLOT;
+        const double* r0 = ring + rslot(it + NS - 1) * TR::SLOT;
+        const double* rm = ring + rslot(it + NS - 2) * TR::SLOT;
+        const double* tzj = tz + (it % NTZ) * PP;
+        mbar_wait(&T->ufull[rslot(it)], rpar(it));      // U*(j) complete
 
-        const bool more = j + 2 <= b.z1;          // E(j+2) exists and needs U(j+3)
-        const bool more_phi = j + 3 <= b.z1;      // C(j+3) exists and needs Phi(j+4)
+        const int kb = j + NS - 2;                // the plane whose bundle (U(kb+1), Phi(kb+2)) takes the freed slot
+        const bool more = kb <= b.z1;             // E(kb) exists
+        const bool more_phi = kb + 1 <= b.z1;     // C(kb+1) exists
 #pragma unroll
         for (int q = 0; q < DROWS; ++q) {
-            const int ty = 2 + dw + NDW * q;
-            const int t = ty * FX + lane;
+            const int t = (2 + dw + NDW * q) * FX + lane;
             LagCoef lc;
             double out[NF];
             bool emit = false;
-            const int xv = b.x0 - 2 + lane, yv = b.y0 - 2 + ty;
-            const bool is_out = lane_out && xv < g.nx && yv < g.ny;
-            const size_t off = (size_t)xv + (size_t)g.nx * yv + (size_t)(j - 1) * nxny;
+            const bool is_out = row_out[q];
+            const size_t off = row_off[q] + (size_t)(j - 1) * nxny;
             // one plane ahead: what this row's NEXT output cell needs from global memory besides the ring
             const double pre = L.pre[q];
             L.pre[q] = TR::early(a, off + nxny, is_out && do_wzp && j + 1 <= b.z1);
@@ -559,23 +571,23 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
             }
             L.Sz_prev[q] = Sz_new;
 
-            // After the last row's lower part ring slot it+2 (plane j-2) is no longer needed by this warp; when
-            // that holds for all of them it takes the bundle of plane j+2: U(j+3) and Phi(j+4)
+            // After the last row's lower part the ring slot of plane j-2 is no longer needed by this warp; when that
+            // holds for all of them it takes the bundle of plane kb = j-2+NS
             if (q == DROWS - 1 && more) {
-                unsigned long long* land = &T->landed[(it + 2) & 3];
-                double* dst = ring + ((it + 2) & 3) * TR::SLOT;
-                double* pdst = phir + ((it + 5) & (NPHI - 1)) * PL;
+                unsigned long long* land = &T->landed[rslot(it + NS - 2)];
+                double* dst = ring + rslot(it + NS - 2) * TR::SLOT;
+                double* pdst = phir + pslot(it + NS + 1) * PL;
                 if (bulk) fence_proxy_async();
                 group_sync(&T->dsync, it & 1);
                 if (bulk) {
                     if (dtid == 0) {
                         mbar_arrive_expect_tx(land, UBYTES + (more_phi ? PBYTES : 0u));
-                        stage_state<TR::NPAIR, TR::LAST1>(a, T, b, dst, j + 3, land, dtid);
-                        if (more_phi) stage_phi(a, T, b, pdst, j + 4, land, dtid);
+                        stage_state<TR::NPAIR, TR::LAST1>(a, T, b, dst, kb + 1, land, dtid);
+                        if (more_phi) stage_phi(a, T, b, pdst, kb + 2, land, dtid);
                     }
                 } else {
-                    stage_state<TR::NPAIR, TR::LAST1>(a, T, b, dst, j + 3, land, dtid);
-                    if (more_phi) stage_phi(a, T, b, pdst, j + 4, land, dtid);
+                    stage_state<TR::NPAIR, TR::LAST1>(a, T, b, dst, kb + 1, land, dtid);
+                    if (more_phi) stage_phi(a, T, b, pdst, kb + 2, land, dtid);
                     mbar_arrive_on_cp_async(land);
                 }
             }
@@ -602,7 +614,7 @@ struct GasTraits {
     static constexpr int NPAIR = 2, NP2 = 0;
     static constexpr bool LAST1 = true;
     static constexpr int SLOT = 2 * PP + PL;
-    static constexpr int PLANES = 2 + 1 + 1 + NPHI + 2 + NS * 5 + 4;
+    static constexpr int PLANES = 2 + 1 + 1 + NPHI + 2 + NS * 5 + 2 * NTZ;
     // density of the other component for the Poisson source, asked for one plane before it is used
     __device__ static __forceinline__ double early(const FusedArgs<NGAS>& a, size_t off, bool is_out) {
         return (a.src_in && is_out) ? a.src_in[BSTR * off] : 0.0;
@@ -647,7 +659,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     const bool bot_dup = !ST && zout && j == 0;
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
-    const double* ph0 = S.phi + ((it + 1) & (NPHI - 1)) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
+    const double* ph0 = S.phi + pslot(it + 1) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
     if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
@@ -691,8 +703,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
 
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
     // publish primitives(j+1)
-    double* rs = S.ring + (it & 3) * GasTraits::SLOT;
-    mbar_wait(&T->landed[it & 3], (it >> 2) & 1);
+    double* rs = S.ring + rslot(it) * GasTraits::SLOT;
+    mbar_wait(&T->landed[rslot(it)], rpar(it));
     const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t);
     const double rho_n = s0.x, mx_n = s0.y, my_n = s1.x, mz_n = s1.y, E_n = rs[2 * PP + t];
     const double ir_n = frcp(rho_n);
@@ -703,11 +715,11 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         gas_face(gamma, c.rho, c.vz, c.p, rho_n, vz_n, p_n, Pz, PVz);
         double wx, wy, wz, Es, dens;
         if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
-            const double* rq = S.ring + ((it + 3) & 3) * GasTraits::SLOT;
+            const double* rq = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
             const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
             dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y; Es = rq[2 * PP + t];
         } else {
-            const double gz = (S.phi[((it + 2) & (NPHI - 1)) * PL + t] - S.phi[(it & (NPHI - 1)) * PL + t]) * inv2h;
+            const double gz = (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h;
             const double trg = tau * c.rho * gz;
             const double mz = c.rho * c.vz;
             const double mzs = c.amz - th2 * Pz - trg;
@@ -716,13 +728,13 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         }
         sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy); rs[2 * PP + t] = Es;
         if (bot_dup) {                        // outflow: U*(-1) := U*(0)
-            double* rg = S.ring + ((it + 3) & 3) * GasTraits::SLOT;
+            double* rg = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
             sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy); rg[2 * PP + t] = Es;
         }
         if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
-            const double2 wm = lds2(S.ring + ((it + 2) & 3) * GasTraits::SLOT + PP + 2 * t);
-            const double2 w0 = lds2(S.ring + ((it + 3) & 3) * GasTraits::SLOT + PP + 2 * t);
-            sts2(S.tz + (it & 1) * PP + 2 * t, sum3(wm.x, w0.x, wx), sum3(wm.y, w0.y, wy));
+            const double2 wm = lds2(S.ring + rslot(it + NS - 2) * GasTraits::SLOT + PP + 2 * t);
+            const double2 w0 = lds2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + PP + 2 * t);
+            sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, w0.x, wx), sum3(wm.y, w0.y, wy));
         }
     }
     sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
@@ -737,18 +749,18 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
             for (int P = 0; P < 2; ++P) {
                 const double2 v = lds2(rs + P * PP + 2 * f.fix_src);
                 sts2(rs + P * PP + 2 * t, v.x, v.y);
-                if (bot_dup) sts2(S.ring + ((it + 3) & 3) * GasTraits::SLOT + P * PP + 2 * t, v.x, v.y);
+                if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + P * PP + 2 * t, v.x, v.y);
             }
             const double e = rs[2 * PP + f.fix_src];
             rs[2 * PP + t] = e;
-            if (bot_dup) S.ring[((it + 3) & 3) * GasTraits::SLOT + 2 * PP + t] = e;
-            const double2 v = lds2(S.tz + (it & 1) * PP + 2 * f.fix_src);
-            sts2(S.tz + (it & 1) * PP + 2 * t, v.x, v.y);
+            if (bot_dup) S.ring[rslot(it + NS - 1) * GasTraits::SLOT + 2 * PP + t] = e;
+            const double2 v = lds2(S.tz + (it % NTZ) * PP + 2 * f.fix_src);
+            sts2(S.tz + (it % NTZ) * PP + 2 * t, v.x, v.y);
         }
         group_sync(&T->esync, 0);
     }
     __syncwarp();
-    if (f.tx == 0) mbar_arrive(&T->ufull[it & 3]);   // this row's U*(j) is complete
+    if (f.tx == 0) mbar_arrive(&T->ufull[rslot(it)]);   // this row's U*(j) is complete
 }
 
 __global__ void __launch_bounds__(NT, 1)
@@ -836,7 +848,7 @@ struct BmeTraits {
     static constexpr int NPAIR = 5, NP2 = 3;
     static constexpr bool LAST1 = false;
     static constexpr int SLOT = 5 * PP;
-    static constexpr int PLANES = 9 + NPHI + 9 + NS * 10 + 4;
+    static constexpr int PLANES = 9 + NPHI + 9 + NS * 10 + 2 * NTZ;
     __device__ static __forceinline__ double early(const FusedArgs<NBME>&, size_t, bool) { return 0.0; }
     __device__ static __forceinline__ void emit(const FusedArgs<NBME>& a, size_t off, const double out[NBME], double, double& smax, int& bad) {
 #pragma unroll
@@ -878,7 +890,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     const bool bot_dup = !ST && zout && j == 0;
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
-    const double* ph0 = S.phi + ((it + 1) & (NPHI - 1)) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
+    const double* ph0 = S.phi + pslot(it + 1) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
     if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
@@ -931,7 +943,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         c.acc[3] -= th4 * (EFy[0] - l1.y); c.acc[4] -= th4 * (EFy[1] - l2.x); c.acc[5] -= th4 * (EFy[2] - l2.y);
         c.acc[6] -= th4 * (EFy[3] - l3.x); c.acc[7] -= th4 * (EFy[4] - l3.y); c.acc[8] -= th4 * (EFy[5] - l4);
         // gravity (reading G5): -tau n g_i and -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
-        const double gr[3] = {gx, gy, (S.phi[((it + 2) & (NPHI - 1)) * PL + t] - S.phi[(it & (NPHI - 1)) * PL + t]) * inv2h};
+        const double gr[3] = {gx, gy, (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h};
         double uc[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], c.u[d]);
@@ -948,8 +960,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
 
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
     // publish primitives(j+1)
-    double* rs = S.ring + (it & 3) * BmeTraits::SLOT;
-    mbar_wait(&T->landed[it & 3], (it >> 2) & 1);
+    double* rs = S.ring + rslot(it) * BmeTraits::SLOT;
+    mbar_wait(&T->landed[rslot(it)], rpar(it));
     double Un[NBME];
     {
         const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t), s2 = lds2(rs + 2 * PP + 2 * t),
@@ -970,7 +982,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         bme_face<2>(c.n, c.u, Pl, n_n, u_n, Pr, Pz, EFz);
         double o[NBME];      // n, w (3), nE (6)
         if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
-            const double* rq = S.ring + ((it + 3) & 3) * BmeTraits::SLOT;
+            const double* rq = S.ring + rslot(it + NS - 1) * BmeTraits::SLOT;
             const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t), q2 = lds2(rq + 2 * PP + 2 * t),
                           q3 = lds2(rq + 3 * PP + 2 * t), q4 = lds2(rq + 4 * PP + 2 * t);
             o[0] = q0.x; o[3] = q0.y; o[1] = q1.x; o[2] = q1.y; o[4] = q2.x; o[5] = q2.y; o[6] = q3.x; o[7] = q3.y;
@@ -985,14 +997,14 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         sts2(rs + 2 * t, o[0], o[3]); sts2(rs + PP + 2 * t, o[1], o[2]); sts2(rs + 2 * PP + 2 * t, o[4], o[5]);
         sts2(rs + 3 * PP + 2 * t, o[6], o[7]); sts2(rs + 4 * PP + 2 * t, o[8], o[9]);
         if (bot_dup) {                        // outflow: U*(-1) := U*(0)
-            double* rg = S.ring + ((it + 3) & 3) * BmeTraits::SLOT;
+            double* rg = S.ring + rslot(it + NS - 1) * BmeTraits::SLOT;
             sts2(rg + 2 * t, o[0], o[3]); sts2(rg + PP + 2 * t, o[1], o[2]); sts2(rg + 2 * PP + 2 * t, o[4], o[5]);
             sts2(rg + 3 * PP + 2 * t, o[6], o[7]); sts2(rg + 4 * PP + 2 * t, o[8], o[9]);
         }
         if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
-            const double2 wm = lds2(S.ring + ((it + 2) & 3) * BmeTraits::SLOT + PP + 2 * t);
-            const double2 w0 = lds2(S.ring + ((it + 3) & 3) * BmeTraits::SLOT + PP + 2 * t);
-            sts2(S.tz + (it & 1) * PP + 2 * t, sum3(wm.x, w0.x, o[1]), sum3(wm.y, w0.y, o[2]));
+            const double2 wm = lds2(S.ring + rslot(it + NS - 2) * BmeTraits::SLOT + PP + 2 * t);
+            const double2 w0 = lds2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + PP + 2 * t);
+            sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, w0.x, o[1]), sum3(wm.y, w0.y, o[2]));
         }
     }
     sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
@@ -1015,15 +1027,15 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
             for (int P = 0; P < 5; ++P) {
                 const double2 v = lds2(rs + P * PP + 2 * f.fix_src);
                 sts2(rs + P * PP + 2 * t, v.x, v.y);
-                if (bot_dup) sts2(S.ring + ((it + 3) & 3) * BmeTraits::SLOT + P * PP + 2 * t, v.x, v.y);
+                if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + P * PP + 2 * t, v.x, v.y);
             }
-            const double2 v = lds2(S.tz + (it & 1) * PP + 2 * f.fix_src);
-            sts2(S.tz + (it & 1) * PP + 2 * t, v.x, v.y);
+            const double2 v = lds2(S.tz + (it % NTZ) * PP + 2 * f.fix_src);
+            sts2(S.tz + (it % NTZ) * PP + 2 * t, v.x, v.y);
         }
         group_sync(&T->esync, 0);
     }
     __syncwarp();
-    if (f.tx == 0) mbar_arrive(&T->ufull[it & 3]);   // this row's U*(j) is complete
+    if (f.tx == 0) mbar_arrive(&T->ufull[rslot(it)]);   // this row's U*(j) is complete
 }
 
 __global__ void __launch_bounds__(NT, 1)
