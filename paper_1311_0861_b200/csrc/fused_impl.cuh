@@ -36,6 +36,8 @@
 // the Poisson mode, so its staging needs no case analysis.
 #include <cuda.h>
 
+#include <cstddef>
+
 #include "gp_internal.h"
 
 namespace gp {
@@ -177,15 +179,24 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, uns
     asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(b)), "r"(bytes)
                  : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+// Wait for the phase of given parity of the mbarrier at shared address base + OFF (bytes; an immediate, so that no
+// second address register stays live across the loop).  try_wait suspends the warp for up to the hinted time, so a
+// waiting warp issues a poll only now and then instead of spinning on the issue port of the working warps.
+template <int OFF = 0>
+__device__ __forceinline__ void mbar_wait_at(unsigned base, unsigned parity) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "W_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%3], %1, %2;\n\t"
         "@p bra D_%=;\n\t"
         "bra W_%=;\n\t"
-        "D_%=:\n\t}" ::"r"(smem_u32(b)), "r"(parity)
+        "D_%=:\n\t}" ::"r"(base), "r"(parity), "r"(0x989680), "n"(OFF)
         : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) { mbar_wait_at<0>(smem_u32(b), parity); }
+template <int OFF = 0>
+__device__ __forceinline__ void mbar_arrive_at(unsigned base) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0+%1];\n\t}" ::"r"(base), "n"(OFF) : "memory");
 }
 // Neighbouring Eulerian warps (footprint rows r, r+1) hand data to each other through two mbarriers per row, one
 // arrival (lane 0 of the producing row) per plane, phase parity = plane parity: yrdy[r] "the y fluxes of row r are
@@ -193,9 +204,10 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
 // r-1 waits before its next stage B).  Each also orders the overwrite that follows it: row r+1 publishes new primitives
 // only after row r has read the old ones, row r rewrites its y fluxes only after row r+1 has read them.  No
 // block-wide barrier is left in the Eulerian group.
-__device__ __forceinline__ void row_arrive(unsigned long long* b) {
+template <int OFF>
+__device__ __forceinline__ void row_arrive_at(unsigned base) {
     __syncwarp();
-    if ((threadIdx.x & 31) == 0) mbar_arrive(b);
+    if ((threadIdx.x & 31) == 0) mbar_arrive_at<OFF>(base);
 }
 // barrier among the warps of one group: one lane per warp arrives, everybody waits for the phase
 __device__ __forceinline__ void group_sync(unsigned long long* b, unsigned parity) {
@@ -253,7 +265,7 @@ __device__ __forceinline__ double sum3_x(double v) { return sum3(from_left(v), v
 // Must be called by whole warps.
 __device__ __forceinline__ double sum9_wz(const double* __restrict__ r, int t) {
     const double2 lo = lds2(r + 2 * (t - FX)), mi = lds2(r + 2 * t), hi = lds2(r + 2 * (t + FX));
-    return sum3(sum3_x(lo.y), sum3_x(mi.y), sum3_x(hi.y));
+    return sum3_x(sum3(lo.y, mi.y, hi.y));       // rows first: one exchange along x instead of three
 }
 
 // Upwind flux form of one cell in coefficient form:
@@ -318,9 +330,8 @@ __device__ __forceinline__ void face_vel_xy(const double* __restrict__ s_tz, int
     const double2 m0 = lds2(s_tz + 2 * (t - FX)), z0 = lds2(s_tz + 2 * t), p0 = lds2(s_tz + 2 * (t + FX));
     const double a_0 = sum3(m0.x, z0.x, p0.x);
     const double a_m = from_left(a_0), a_p = from_right(a_0);
-    const double b_m = sum3_x(m0.y), b_0 = sum3_x(z0.y), b_p = sum3_x(p0.y);
     wxm = a_m + a_0; wxp = a_0 + a_p;
-    wym = b_m + b_0; wyp = b_0 + b_p;
+    wym = sum3_x(m0.y + z0.y); wyp = sum3_x(z0.y + p0.y);   // the two-row sums first: two exchanges along x instead of three
 }
 
 // tensor maps of a launch: the field pairs (then the gas energy) of U, and the padded Phi
@@ -459,9 +470,15 @@ struct Foot {
     size_t base, nxny;
     bool star_row, fix;
     int fix_src;
+    unsigned tabbar;     // shared address of the block table (= of landed[0])
+    unsigned rowbar;     // shared address of yrdy[ty - 1]; the row's other hand-off barriers sit at the offsets below
 };
+// byte offsets from Foot::rowbar: y fluxes of the row below / of this row, primitives of this row / of the row above
+constexpr int OY_LO = 0, OY_OWN = 8, OP_OWN = 8 + 8 * FY, OP_UP = 16 + 8 * FY;
+static_assert(offsetof(BlockTab, landed) == 0 && offsetof(BlockTab, ufull) == 8 * NS, "ring barriers are addressed from the table base");
+static_assert(offsetof(BlockTab, prdy) == offsetof(BlockTab, yrdy) + 8 * FY, "row barriers are addressed from yrdy");
 
-__device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b) {
+__device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b, const BlockTab* T) {
     Foot f;
     f.tx = threadIdx.x & 31; f.ty = threadIdx.x >> 5; f.t = f.ty * FX + f.tx;
     f.xv = b.x0 - 2 + f.tx; f.yv = b.y0 - 2 + f.ty;
@@ -479,6 +496,8 @@ __device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b) {
         else if (f.yv == g.ny) { f.fix_src -= FX; f.fix = true; }
     }
     f.fix = f.fix && f.star_row && f.tx >= 1 && f.tx <= FX - 2;
+    f.tabbar = smem_u32(T);
+    f.rowbar = smem_u32(&T->yrdy[0]) + 8 * (f.ty - 1);
     return f;
 }
 
@@ -660,7 +679,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
     const double* ph0 = S.phi + pslot(it + 1) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
-    if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
+    if (it > 0 && f.ty < FY - 1) mbar_wait_at<OP_UP>(f.rowbar, (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
     // that the two solvers interleave
@@ -689,8 +708,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         gas_face(gamma, c.rho, c.vy, c.p, ry.x, S.vy[t + FX], ry.y, Pyh, PVyh);
         sts2(S.fy + 2 * t, Pyh, PVyh);
     }
-    row_arrive(&T->yrdy[f.ty]);                                  // y fluxes of this row are written
-    if (f.ty > 0) mbar_wait(&T->yrdy[f.ty - 1], it & 1);       // ... and those of the row below
+    row_arrive_at<OY_OWN>(f.rowbar);                                  // y fluxes of this row are written
+    if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);       // ... and those of the row below
 
     // C: y-flux difference
     if (f.star_row) {
@@ -704,7 +723,8 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
     // publish primitives(j+1)
     double* rs = S.ring + rslot(it) * GasTraits::SLOT;
-    mbar_wait(&T->landed[rslot(it)], rpar(it));
+    const unsigned slotbar = f.tabbar + 8 * rslot(it);
+    mbar_wait_at<0>(slotbar, rpar(it));
     const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t);
     const double rho_n = s0.x, mx_n = s0.y, my_n = s1.x, mz_n = s1.y, E_n = rs[2 * PP + t];
     const double ir_n = frcp(rho_n);
@@ -740,7 +760,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
     c.amx = mx_n; c.amy = my_n; c.amz = fma(th2, Pz, mz_n); c.aE = fma(th4, PVz, E_n);
     c.rho = rho_n; c.ir = ir_n; c.vx = vx_n; c.vy = vy_n; c.vz = vz_n; c.p = p_n;
-    row_arrive(&T->prdy[f.ty]);                                  // primitives of plane j+1 of this row are published
+    row_arrive_at<OP_OWN>(f.rowbar);                                  // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
@@ -760,7 +780,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         group_sync(&T->esync, 0);
     }
     __syncwarp();
-    if (f.tx == 0) mbar_arrive(&T->ufull[rslot(it)]);   // this row's U*(j) is complete
+    if (f.tx == 0) mbar_arrive_at<8 * NS>(slotbar);   // this row's U*(j) is complete
 }
 
 __global__ void __launch_bounds__(NT, 1)
@@ -801,7 +821,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
 #endif
-        const Foot f = make_foot(g, b);
+        const Foot f = make_foot(g, b, T);
         const int t = f.t;
         GasCarry c;
         {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
@@ -891,7 +911,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     const bool do_out = ST || j - 1 >= b.z0;
     const int it = j - (b.z0 - 1);
     const double* ph0 = S.phi + pslot(it + 1) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
-    if (it > 0 && f.ty < FY - 1) mbar_wait(&T->prdy[f.ty + 1], (it - 1) & 1);   // primitives of plane j of the row above are published
+    if (it > 0 && f.ty < FY - 1) mbar_wait_at<OP_UP>(f.rowbar, (it - 1) & 1);   // primitives of plane j of the row above are published
 
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
     // dependent chains interleave
@@ -931,8 +951,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
         fy[4 * PP + t] = EFy[5];
     }
-    row_arrive(&T->yrdy[f.ty]);                                  // y fluxes of this row are written
-    if (f.ty > 0) mbar_wait(&T->yrdy[f.ty - 1], it & 1);       // ... and those of the row below
+    row_arrive_at<OY_OWN>(f.rowbar);                                  // y fluxes of this row are written
+    if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);       // ... and those of the row below
 
     // C: y-flux difference, then everything of U*(j) but the upper z face
     if (f.star_row) {
@@ -961,7 +981,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
     // publish primitives(j+1)
     double* rs = S.ring + rslot(it) * BmeTraits::SLOT;
-    mbar_wait(&T->landed[rslot(it)], rpar(it));
+    const unsigned slotbar = f.tabbar + 8 * rslot(it);
+    mbar_wait_at<0>(slotbar, rpar(it));
     double Un[NBME];
     {
         const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t), s2 = lds2(rs + 2 * PP + 2 * t),
@@ -1018,7 +1039,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     for (int d = 0; d < 3; ++d) c.u[d] = u_n[d];
 #pragma unroll
     for (int q = 0; q < 6; ++q) c.Pi[q] = Pi_n[q];
-    row_arrive(&T->prdy[f.ty]);                                  // primitives of plane j+1 of this row are published
+    row_arrive_at<OP_OWN>(f.rowbar);                                  // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
@@ -1035,7 +1056,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         group_sync(&T->esync, 0);
     }
     __syncwarp();
-    if (f.tx == 0) mbar_arrive(&T->ufull[rslot(it)]);   // this row's U*(j) is complete
+    if (f.tx == 0) mbar_arrive_at<8 * NS>(slotbar);   // this row's U*(j) is complete
 }
 
 __global__ void __launch_bounds__(NT, 1)
@@ -1076,7 +1097,7 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
 #endif
-        const Foot f = make_foot(g, b);
+        const Foot f = make_foot(g, b, T);
         const int t = f.t;
         BmeCarry c;
         {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
