@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — cell-updates/s per full timestep (fp64) of the GPUPEGAS hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 512] [--poisson periodic|isolated]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 512] [--poisson periodic|isolated] [--od]
 
 A "step" is one pass of the whole hot path over the synthetic workload: gp_max_dt (device-resident
 dt) + gp_solve_poisson + gp_step.  Default workload = BASELINE.json config 5 (two-galaxy collision,
@@ -250,9 +250,16 @@ def run_gpu(args):
     # inputs: generated on the host (seeded, synthetic) into pinned buffers, handed over through the C ABI
     host = {k: torch.empty((w.nz, w.ny, w.nx), dtype=torch.float64, pin_memory=True) for k in names}
     w.fill({k: v.numpy() for k, v in host.items()})
-    sim = pkg.Simulation.from_workload(w)
+    if args.od:
+        # the same workload carrying the overdetermined system: rho*eps and Pi_ij ride in the fused
+        # kernels, kappa and the energy balance in their epilogues; not the headline (BASELINE.json names the base step)
+        sim = pkg.Simulation(w.nx, w.ny, w.nz, w.h, w.components | pkg.binding.GP_OD, w.poisson, w.G, w.gamma, w.bc)
+    else:
+        sim = pkg.Simulation.from_workload(w)
     for k in names:
         sim.set(k, host[k].numpy())
+    if args.od:
+        sim.od_derive()
     sim.synchronize()
     t_setup = time.perf_counter() - t_setup
 
@@ -310,6 +317,8 @@ def run_gpu(args):
     def e2e_step():
         for k in names:
             sim.set(k, host[k].numpy())            # H2D inside the timed region
+        if args.od:
+            sim.od_derive()
         sim.max_dt(w.cfl)                          # dt comes back to the host
         if gravity:
             sim.solve_poisson()
@@ -339,10 +348,12 @@ def run_gpu(args):
     top = max(own, key=lambda k: own[k][0])
     top_ms = own[top][0] / own[top][1]
     algo = ALGO_BYTES_PER_CELL.get(top, 0) * cells
+    if args.od and top.startswith("hydro_"):   # one / six more fields each way
+        algo += 2 * W * cells * (1 if top == "hydro_gas_fused" else 6)
     if not gravity and top.startswith("hydro_"):
         algo -= W * cells                      # no Phi to read without gravity
     achieved = algo / (top_ms * 1e-3) / 1e9
-    wkey = f"{w.name}_{w.nx}_{args.poisson if gravity else 'nogravity'}"
+    wkey = f"{w.name}_{w.nx}_{args.poisson if gravity else 'nogravity'}" + ("_od" if args.od else "")
     roofline = {"bound": "hbm", "kernel": top, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": stored_traffic(top, wkey), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": algo, "ms_per_launch": top_ms}
@@ -359,6 +370,8 @@ def run_gpu(args):
                         "peak_source": "148 SMs x 64 fp64 lanes (ncu pipe peak, DESIGN.md 8) x max SM clock",
                         "peak_selftest": rate / 1e12}
     step_bytes = STEP_BYTES_PER_CELL[step_bytes_key(w)]
+    if args.od:
+        step_bytes += 2 * W * ((1 if w.components & wl.GAS else 0) + (6 if w.components & wl.STARS else 0))
     per_gpu = value / world
     step_roofline = {"bytes_per_cell_step": step_bytes,
                      "frac_of_8TBs": per_gpu * step_bytes / 8.0e12,
@@ -375,7 +388,7 @@ def run_gpu(args):
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": wname, "grid": [w.nx, w.ny, w.nz], "components": "+".join(k for k in step_bytes_key(w) if k in ("gas", "stars")), "poisson": args.poisson if gravity else "none",
-                   "cfl": w.cfl, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                   "overdetermined": bool(args.od), "cfl": w.cfl, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                    "cache": (f"inputs larger than L2: {len(names) * cells * W / 1e9:.1f} GB of state per step vs 126 MB L2 (no flush)"
                              if len(names) * cells * W > 4 * 126e6 else "state fits in L2 (latency-bound case, not a bandwidth measurement)"),
                    "timing": f"median of {args.repeats} repeats of {args.steps} steps, CUDA events on the library's stream, no per-kernel events inside",
@@ -408,6 +421,8 @@ def main():
     ap.add_argument("--selftest-peak", action="store_true",
                     help="run the DFMA self test that backs the fp64 peak of roofline_alu, print it and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--od", action="store_true",
+                    help="carry the overdetermined system (GP_OD context: rho*eps, Pi_ij, kappa, energy balance); the CPU legs stay the base scheme")
     args = ap.parse_args()
     if args.config == 3:
         args.poisson = "isolated"

@@ -35,21 +35,27 @@ typedef struct gp_ctx gp_ctx;   /* opaque; created by gp_create, freed by gp_des
 enum { GP_OK = 0, GP_ERR_ARG = 1, GP_ERR_ALLOC = 2, GP_ERR_CUDA = 3, GP_ERR_CUFFT = 4,
        GP_ERR_STATE = 5 /* NaN/Inf, or rho, n, p or Pi_dd <= 0 seen */, GP_ERR_UNSUPPORTED = 6 };
 
-enum { GP_GAS = 1, GP_STARS = 2 };                                  /* components bit mask */
+/* components bit mask.  GP_OD: carry the overdetermined system of the paper as well (see below). */
+enum { GP_GAS = 1, GP_STARS = 2, GP_OD = 4 };
 enum { GP_POISSON_NONE = 0, GP_POISSON_PERIODIC = 1, GP_POISSON_ISOLATED = 2 };
 enum { GP_BC_PERIODIC = 0, GP_BC_OUTFLOW = 1 };
 
 /* Conserved fields.  Gas: rho, rho*v (3), rho*E.  Collisionless component
  * (PAPER.md:57, 63): n, n*u (3), n*E_ij (6, symmetric: xx xy xz yy yz zz).  Potential
- * (PAPER.md:186): Phi + Phi0, one field for the summed density. */
+ * (PAPER.md:186): Phi + Phi0, one field for the summed density.  gp_set_state / gp_get_state take any of these
+ * ids (GP_EPS ... GP_PZZ only on a GP_OD context). */
 enum { GP_RHO = 0, GP_MX, GP_MY, GP_MZ, GP_E,
        GP_N, GP_NUX, GP_NUY, GP_NUZ, GP_EXX, GP_EXY, GP_EXZ, GP_EYY, GP_EYZ, GP_EZZ,
-       GP_PHI, GP_NFIELDS };
+       GP_PHI, GP_NFIELDS,
+       /* Carried fields of the overdetermined system (contexts created with GP_OD only): the internal energy
+        * rho*eps of the gas (4th equation) and the velocity-dispersion tensor Pi_ij of the
+        * collisionless component (xx xy xz yy yz zz). */
+       GP_EPS = GP_NFIELDS, GP_PXX, GP_PXY, GP_PXZ, GP_PYY, GP_PYZ, GP_PZZ, GP_NFIELDS_OD };
 
 typedef struct {
     int nx, ny, nz;      /* interior cells per axis */
     double h;            /* cell size (with h_x = h_y = h_z) */
-    int components;      /* GP_GAS | GP_STARS */
+    int components;      /* GP_GAS | GP_STARS [| GP_OD] */
     int poisson;         /* GP_POISSON_* */
     double G;            /* gravitational constant multiplying the source of PAPER.md:186 */
 } gp_grid;
@@ -93,6 +99,37 @@ int gp_max_dt(gp_ctx* ctx, double cfl, double* dt);
  * flux-form advection), for every enabled component.  dt > 0: use it; dt <= 0: use the
  * device-resident dt of the last gp_max_dt. */
 int gp_step(gp_ctx* ctx, double dt);
+
+/* ---- overdetermined system and correctness check (contexts created with GP_OD) ----
+ * Besides rho*E and n*E_ij the scheme carries rho*eps (4th equation) and Pi_ij by their
+ * own equations.  In a GP_OD context both stages take the pressure p = (gamma-1) rho*eps and the dispersion tensor
+ * from the CARRIED fields; the Eulerian stage also updates them,
+ *     (rho eps)* = rho eps - tau (gamma-1) rho eps  sum_d (V_{d+1/2} - V_{d-1/2}) / h,
+ *     Pi_ij*     = Pi_ij   - tau sum_k [Pi_jk (u*_i|_{k+1/2} - u*_i|_{k-1/2}) + Pi_ik (u*_j|_{k+1/2} - u*_j|_{k-1/2})] / h
+ * with the face values V, u* of PAPER.md:112 and 170-172, and the Lagrangian stage advects them like every other
+ * field.  All other GP_OD calls return GP_ERR_UNSUPPORTED on a context created without GP_OD.
+ *
+ * gp_od_derive: carried fields := what the conserved fields imply (rho eps = rho E - rho v^2/2, PAPER.md:41 last
+ *   line; Pi_ij = n E_ij - n u_i u_j).  Call it after setting the conserved fields, unless the
+ *   carried fields are set explicitly with gp_set_state(GP_EPS ... GP_PZZ).
+ * gp_od_step: one timestep as above; dt as in gp_step.  balance != 0 applies the energy balance (below) to the new
+ *   state inside the same kernels.  gp_step on a GP_OD context is gp_od_step(ctx, dt, 1).
+ * gp_od_balance: the "energy balance procedure" (PAPER.md:202 only cites it; reading G15 -- this build's
+ *   own design), cell by cell on the current state: where rho E - rho v^2/2 > 0 (all three Pi_dd of
+ *   n E_ij - n u_i u_j > 0) the total-energy description wins and the carried field is reset from it; elsewhere the
+ *   carried field wins: |v| is rescaled, direction kept, so that rho v^2/2 = rho E - rho eps (v := 0 and
+ *   rho E := rho eps if even that is not positive), and n E_ij := Pi_ij + n u_i u_j.
+ * gp_kappa: out[0] = kappa_gas = sum |rho E - rho eps - rho v^2/2| h^3, out[1] = kappa_bme = sum over the six
+ *   components of |n E_ij - Pi_ij - n u_i u_j| h^3 of the CURRENT state (host pointer;
+ *   synchronises).  A component that is not enabled reports 0.
+ * gp_od_last_kappa: the same two sums for the state the last gp_od_step / gp_step produced BEFORE its balance was
+ *   applied, folded by the step kernels at no extra pass (the paper's per-step check); GP_ERR_STATE if no step has
+ *   run since the state was last set. */
+int gp_od_derive(gp_ctx* ctx);
+int gp_od_step(gp_ctx* ctx, double dt, int balance);
+int gp_od_balance(gp_ctx* ctx);
+int gp_kappa(gp_ctx* ctx, double* out);
+int gp_od_last_kappa(gp_ctx* ctx, double* out);
 
 const char* gp_last_error(void);   /* thread-local static text; never freed by the caller */
 

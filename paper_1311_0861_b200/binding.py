@@ -11,19 +11,21 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libgpupegas.so")
 
 GP_OK, GP_ERR_ARG, GP_ERR_ALLOC, GP_ERR_CUDA, GP_ERR_CUFFT, GP_ERR_STATE, GP_ERR_UNSUPPORTED = range(7)
-GP_GAS, GP_STARS = 1, 2
+GP_GAS, GP_STARS, GP_OD = 1, 2, 4
 GP_POISSON_NONE, GP_POISSON_PERIODIC, GP_POISSON_ISOLATED = 0, 1, 2
 GP_BC_PERIODIC, GP_BC_OUTFLOW = 0, 1
 FIELDS = ["rho", "mx", "my", "mz", "E",
           "n", "nux", "nuy", "nuz", "Exx", "Exy", "Exz", "Eyy", "Eyz", "Ezz", "phi"]
-FIELD_ID = {name: i for i, name in enumerate(FIELDS)}
+# carried fields of the overdetermined system (GP_OD contexts): GP_EPS, GP_PXX ... GP_PZZ
+OD_GAS_FIELDS, OD_STAR_FIELDS = ["eps"], ["Pxx", "Pxy", "Pxz", "Pyy", "Pyz", "Pzz"]
+FIELD_ID = {name: i for i, name in enumerate(FIELDS + OD_GAS_FIELDS + OD_STAR_FIELDS)}
 GAS_FIELDS, STAR_FIELDS = FIELDS[:5], FIELDS[5:15]
 
 # the symbols include/gpupegas.h declares
 EXPORTS = ["gp_create", "gp_destroy", "gp_set_state", "gp_get_state", "gp_solve_poisson", "gp_max_dt",
            "gp_step", "gp_last_error", "gp_set_stream", "gp_storage_bytes", "gp_bind_storage",
            "gp_synchronize", "gp_launch_counts", "gp_timing_enable", "gp_timing_read", "gp_math_selftest",
-           "gp_fp64_rate_selftest"]
+           "gp_fp64_rate_selftest", "gp_od_derive", "gp_od_step", "gp_od_balance", "gp_kappa", "gp_od_last_kappa"]
 
 
 class gp_grid(C.Structure):
@@ -73,6 +75,11 @@ def lib():
         L.gp_timing_read.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_char_p), dp, C.POINTER(C.c_longlong)]
         L.gp_math_selftest.argtypes = [C.c_int, vp, vp, vp]
         L.gp_fp64_rate_selftest.argtypes = [dp, dp]
+        L.gp_od_derive.argtypes = [vp]
+        L.gp_od_step.argtypes = [vp, C.c_double, C.c_int]
+        L.gp_od_balance.argtypes = [vp]
+        L.gp_kappa.argtypes = [vp, dp]
+        L.gp_od_last_kappa.argtypes = [vp, dp]
         _lib = L
     return _lib
 
@@ -144,6 +151,12 @@ class Simulation:
     def field_names(self):
         return (GAS_FIELDS if self.components & GP_GAS else []) + (STAR_FIELDS if self.components & GP_STARS else [])
 
+    def od_field_names(self):
+        """The carried fields of a GP_OD context."""
+        if not self.components & GP_OD:
+            return []
+        return (OD_GAS_FIELDS if self.components & GP_GAS else []) + (OD_STAR_FIELDS if self.components & GP_STARS else [])
+
     # ---- state in / out -------------------------------------------------------------------
     def set(self, name, arr):
         """arr: numpy float64 array (host) or a torch float64 CUDA tensor of nz*ny*nx elements."""
@@ -192,6 +205,28 @@ class Simulation:
     def step(self, dt=0.0):
         """dt > 0: use it; dt <= 0: use the device-resident dt of the last max_dt."""
         _chk(lib().gp_step(self._c, dt), "gp_step")
+
+    # ---- overdetermined system (GP_OD contexts) -------------------------------------------
+    def od_derive(self):
+        _chk(lib().gp_od_derive(self._c), "gp_od_derive")
+
+    def od_step(self, dt=0.0, balance=True):
+        _chk(lib().gp_od_step(self._c, dt, 1 if balance else 0), "gp_od_step")
+
+    def od_balance(self):
+        _chk(lib().gp_od_balance(self._c), "gp_od_balance")
+
+    def kappa(self):
+        """(kappa_gas, kappa_bme) of the current state."""
+        out = (C.c_double * 2)()
+        _chk(lib().gp_kappa(self._c, out), "gp_kappa")
+        return out[0], out[1]
+
+    def od_last_kappa(self):
+        """(kappa_gas, kappa_bme) of the state the last step produced, before its balance."""
+        out = (C.c_double * 2)()
+        _chk(lib().gp_od_last_kappa(self._c, out), "gp_od_last_kappa")
+        return out[0], out[1]
 
     def synchronize(self):
         _chk(lib().gp_synchronize(self._c), "gp_synchronize")

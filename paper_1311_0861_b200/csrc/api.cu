@@ -23,7 +23,7 @@ static const char* const kKernelNames[K_NUM] = {
     "cfl", "poisson_source", "cufft_forward",
     "poisson_green", "cufft_inverse", "phi_ghost", "poisson_pad_source", "poisson_mul_kernel", "poisson_extract",
     "hydro_gas_fused", "hydro_bme_fused", "poisson_zpass_green", "poisson_iso_yfwd", "poisson_iso_zfused",
-    "poisson_iso_yinv"};
+    "poisson_iso_yinv", "od_cell_local"};
 
 void tic(gp_ctx* c, int kid) {
     Timing* t = c->tim;
@@ -65,7 +65,11 @@ static void timing_collect(gp_ctx* c) {
 
 static bool field_enabled(const gp_grid& g, int f) {
     if (f == GP_PHI) return true;
-    if (f < 0 || f >= GP_NFIELDS) return false;
+    if (f < 0 || f >= GP_NFIELDS_OD) return false;
+    if (f >= GP_EPS) {
+        if (!(g.components & GP_OD)) return false;
+        return f == GP_EPS ? (g.components & GP_GAS) != 0 : (g.components & GP_STARS) != 0;
+    }
     return f < NGAS ? (g.components & GP_GAS) != 0 : (g.components & GP_STARS) != 0;
 }
 
@@ -73,11 +77,12 @@ static size_t storage_bytes(const gp_grid& g) {
     const size_t N = (size_t)g.nx * g.ny * g.nz;
     const size_t fb = align256(N * sizeof(double));
     size_t nf = 0;
-    if (g.components & GP_GAS) nf += NGAS;
-    if (g.components & GP_STARS) nf += NBME;
-    size_t b = 2 * nf * fb;                           // U and the step's target
+    const bool od = (g.components & GP_OD) != 0;
+    if (g.components & GP_GAS) nf += NGAS + (od ? NODG : 0);
+    if (g.components & GP_STARS) nf += NBME + (od ? NODB : 0);
+    size_t b = 2 * nf * fb + 64 * 256;                // U and the step's target (pairs are aligned one by one)
     b += align256(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double));   // Phi with two ghost layers
-    b += 256;                                         // dt, smax, flag
+    b += 512;                                         // dt, smax, flag; kappa
     b += poisson_storage_bytes(&g);
     return b;
 }
@@ -104,7 +109,19 @@ static int ensure_storage(gp_ctx* c) {
     char* p = c->base;
     auto take = [&](size_t bytes) { char* r = p; p += align256(bytes); return r; };
     const size_t N = c->N;
-    for (int f = 0; f < NHYD; ++f) c->U[f] = c->Us[f] = nullptr;
+    for (int f = 0; f < NALL; ++f) c->U[f] = c->Us[f] = nullptr;
+    c->od = (g.components & GP_OD) != 0;
+    c->estr = c->od ? BSTR : 1;
+    auto take_pair = [&](int f0, int f1) {            // one double2 per cell (gp_internal.h, BSTR)
+        double* u = (double*)take(2 * N * sizeof(double));
+        double* us = (double*)take(2 * N * sizeof(double));
+        c->U[f0] = u; c->U[f1] = u + 1;
+        c->Us[f0] = us; c->Us[f1] = us + 1;
+    };
+    if (c->od) {
+        if (g.components & GP_GAS) take_pair(NGAS - 1, F_EPS);                      // (rho E, rho eps)
+        if (g.components & GP_STARS) for (int P = 0; P < NODB / 2; ++P) take_pair(F_PI + 2 * P, F_PI + 2 * P + 1);
+    }
     if (g.components & GP_GAS) {
         for (int P = 0; P < NGASP / 2; ++P) {     // (rho,m_x) (m_y,m_z): one double2 per cell (gp_internal.h, BSTR)
             double* u = (double*)take(2 * N * sizeof(double));
@@ -112,8 +129,10 @@ static int ensure_storage(gp_ctx* c) {
             c->U[2 * P] = u; c->U[2 * P + 1] = u + 1;
             c->Us[2 * P] = us; c->Us[2 * P + 1] = us + 1;
         }
-        c->U[GP_E] = (double*)take(N * sizeof(double));
-        c->Us[GP_E] = (double*)take(N * sizeof(double));
+        if (!c->od) {
+            c->U[GP_E] = (double*)take(N * sizeof(double));
+            c->Us[GP_E] = (double*)take(N * sizeof(double));
+        }
     }
     if (g.components & GP_STARS)
         for (int P = 0; P < NBME / 2; ++P) {      // pairs of fields, one double2 per cell (gp_internal.h, BSTR)
@@ -123,6 +142,8 @@ static int ensure_storage(gp_ctx* c) {
             c->Us[NGAS + 2 * P] = us; c->Us[NGAS + 2 * P + 1] = us + 1;
         }
     c->phip = (double*)take(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double));
+    c->d_kappa = (double*)take(256);
+    c->kappa_cached = false;
     char* small = take(256);
     c->d_dt = (double*)small;
     c->d_smax = (unsigned long long*)(small + 64);
@@ -195,8 +216,8 @@ gp_ctx* gp_create(const gp_grid* grid, double gamma, const gp_bc* bc) {
         set_error("gp_create: need nx, ny, nz >= 4 and h > 0");
         return nullptr;
     }
-    if (!(grid->components & (GP_GAS | GP_STARS)) || (grid->components & ~(GP_GAS | GP_STARS))) {
-        set_error("gp_create: components must be GP_GAS, GP_STARS or both");
+    if (!(grid->components & (GP_GAS | GP_STARS)) || (grid->components & ~(GP_GAS | GP_STARS | GP_OD))) {
+        set_error("gp_create: components must be GP_GAS, GP_STARS or both, optionally with GP_OD");
         return nullptr;
     }
     if (grid->poisson < GP_POISSON_NONE || grid->poisson > GP_POISSON_ISOLATED) { set_error("gp_create: bad poisson mode"); return nullptr; }
@@ -320,13 +341,14 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
         if ((rc = copy_phi(c, const_cast<double*>(src), on_device != 0, true)) != GP_OK) return rc;
         return launch_phi_ghost_bc(c, c->bc.x, c->bc.y, c->bc.z);
     }
-    double* dst = c->U[field];
-    if (field_paired(field)) {
+    const int fi = field_index(field);
+    double* dst = c->U[fi];
+    if (field_paired(fi, c->od)) {
         // paired layout: a host array lands contiguously in the pair's step target (free between steps),
         // then one kernel interleaves it; a device array is interleaved directly
         const double* from = src;
         if (!on_device) {
-            double* scratch = c->Us[pair_base(field)];
+            double* scratch = c->Us[pair_base(fi)];
             GP_CUDA(cudaMemcpyAsync(scratch, src, c->N * sizeof(double), cudaMemcpyHostToDevice, c->stream));
             GP_CUDA(cudaStreamSynchronize(c->stream));
             from = scratch;
@@ -338,6 +360,7 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     }
     c->cfl_cached = false;
     c->src_cached = false;
+    c->kappa_cached = false;
     return GP_OK;
 }
 
@@ -347,9 +370,10 @@ int gp_get_state(gp_ctx* c, int field, double* dst, int on_device) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     if (field == GP_PHI) return copy_phi(c, dst, on_device != 0, false);
-    const double* src = c->U[field];
-    if (field_paired(field)) {
-        double* scratch = c->Us[pair_base(field)];
+    const int fi = field_index(field);
+    const double* src = c->U[fi];
+    if (field_paired(fi, c->od)) {
+        double* scratch = c->Us[pair_base(fi)];
         if ((rc = launch_strided_copy(c, on_device ? dst : scratch, 1, src, BSTR, c->N)) != GP_OK) return rc;
         if (!on_device) {
             GP_CUDA(cudaMemcpyAsync(dst, scratch, c->N * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -389,28 +413,91 @@ int gp_max_dt(gp_ctx* c, double cfl, double* dt) {
     return GP_OK;
 }
 
-int gp_step(gp_ctx* c, double dt) {
-    if (!c) { set_error("gp_step: NULL context"); return GP_ERR_ARG; }
-    if (dt != dt) { set_error("gp_step: dt is NaN"); return GP_ERR_ARG; }
+// One timestep; od_balance: -1 = plain scheme, 0 / 1 = overdetermined system without / with the energy balance.
+static int step_impl(gp_ctx* c, double dt, int od_balance) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
+    const bool od = od_balance >= 0;
     const double* d_dt = dt > 0.0 ? nullptr : c->d_dt;
     if ((rc = launch_cfl_reset_next(c)) != GP_OK) return rc;
+    if (od) GP_CUDA(cudaMemsetAsync(c->d_kappa, 0, 2 * sizeof(double), c->stream));
+    auto swap = [&](int f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; };
     // With both components and the periodic solve, the source rho + n of the next solve rides in
     // the epilogue of the gas kernel, which therefore runs second (n is then already new).
     c->src_cached = false;
     if (c->g.components & GP_STARS) {
-        if ((rc = launch_fused_bme(c, dt, d_dt)) != GP_OK) return rc;
-        for (int f = NGAS; f < NHYD; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
+        if ((rc = od ? launch_fused_bme_od(c, dt, d_dt, od_balance) : launch_fused_bme(c, dt, d_dt)) != GP_OK) return rc;
+        for (int f = NGAS; f < NHYD; ++f) swap(f);
+        if (od) for (int f = F_PI; f < NALL; ++f) swap(f);
     }
     if (c->g.components & GP_GAS) {
         double* src_out = c->src;          // non-null only with the periodic solve
         const double* n_new = (c->g.components & GP_STARS) ? c->U[GP_N] : nullptr;
-        if ((rc = launch_fused_gas(c, dt, d_dt, src_out ? n_new : nullptr, src_out)) != GP_OK) return rc;
-        for (int f = 0; f < NGAS; ++f) { double* t = c->U[f]; c->U[f] = c->Us[f]; c->Us[f] = t; }
+        if ((rc = od ? launch_fused_gas_od(c, dt, d_dt, src_out ? n_new : nullptr, src_out, od_balance)
+                     : launch_fused_gas(c, dt, d_dt, src_out ? n_new : nullptr, src_out)) != GP_OK) return rc;
+        for (int f = 0; f < NGAS; ++f) swap(f);
+        if (od) swap(F_EPS);
         c->src_cached = src_out != nullptr;
     }
     c->cfl_cached = true;
+    c->kappa_cached = od;
+    return GP_OK;
+}
+
+int gp_step(gp_ctx* c, double dt) {
+    if (!c) { set_error("gp_step: NULL context"); return GP_ERR_ARG; }
+    if (dt != dt) { set_error("gp_step: dt is NaN"); return GP_ERR_ARG; }
+    return step_impl(c, dt, (c->g.components & GP_OD) ? 1 : -1);
+}
+
+#define GP_NEED_OD(name)                                                                                  \
+    do {                                                                                                  \
+        if (!c) { set_error(name ": NULL context"); return GP_ERR_ARG; }                                  \
+        if (!(c->g.components & GP_OD)) { set_error(name ": context was created without GP_OD"); return GP_ERR_UNSUPPORTED; } \
+    } while (0)
+
+int gp_od_step(gp_ctx* c, double dt, int balance) {
+    GP_NEED_OD("gp_od_step");
+    if (dt != dt) { set_error("gp_od_step: dt is NaN"); return GP_ERR_ARG; }
+    return step_impl(c, dt, balance ? 1 : 0);
+}
+
+int gp_od_derive(gp_ctx* c) {
+    GP_NEED_OD("gp_od_derive");
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    c->kappa_cached = false;
+    return launch_od_derive(c);
+}
+
+int gp_od_balance(gp_ctx* c) {
+    GP_NEED_OD("gp_od_balance");
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    c->cfl_cached = false;       // the balance may change momenta and energies
+    c->kappa_cached = false;
+    return launch_od_balance(c);
+}
+
+int gp_kappa(gp_ctx* c, double* out) {
+    GP_NEED_OD("gp_kappa");
+    if (!out) { set_error("gp_kappa: NULL argument"); return GP_ERR_ARG; }
+    int rc = ensure_storage(c);
+    if (rc != GP_OK) return rc;
+    if ((rc = launch_od_kappa(c, c->d_kappa + 2)) != GP_OK) return rc;
+    GP_CUDA(cudaMemcpyAsync(out, c->d_kappa + 2, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    GP_CUDA(cudaStreamSynchronize(c->stream));
+    return GP_OK;
+}
+
+int gp_od_last_kappa(gp_ctx* c, double* out) {
+    GP_NEED_OD("gp_od_last_kappa");
+    if (!out) { set_error("gp_od_last_kappa: NULL argument"); return GP_ERR_ARG; }
+    if (!c->ready || !c->kappa_cached) { set_error("gp_od_last_kappa: no step has run since the state was last set"); return GP_ERR_STATE; }
+    GP_CUDA(cudaMemcpyAsync(out, c->d_kappa, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    GP_CUDA(cudaStreamSynchronize(c->stream));
+    const double h3 = c->g.h * c->g.h * c->g.h;
+    out[0] *= h3; out[1] *= h3;
     return GP_OK;
 }
 

@@ -1,0 +1,13 @@
+// Fused hydro step of the collisionless component carrying the overdetermined system (GP_OD contexts;
+// fused_impl.cuh with GP_OVERDET): sixteen fields (Pi_ij as three more pairs).  The ring alone takes 64 planes, so the
+// footprint is 32 x 8 cells (95 planes, 190 KB): eight Eulerian warps and four Lagrangian warps (384 threads launched
+// at 168 registers, re-split with setmaxnreg).
+#define GP_OVERDET 1
+#define GP_NS 4
+#define GP_FY 8
+#define GP_NDW 4
+#define GP_REG_E 200
+#define GP_REG_D 104
+#define GP_FUSED_NS fbmeod
+#define GP_FUSED_BME 1
+#include "fused_impl.cuh"

@@ -1,12 +1,13 @@
-// Fused hydro step of the gas (fused_impl.cuh): footprint of 32 x 16 cells, sixteen Eulerian warps and four
-// Lagrangian warps (640 threads, 96 registers each).
+// Fused hydro step of the gas (fused_impl.cuh): footprint of 32 x 16 cells, sixteen Eulerian warps and
+// twelve single-row Lagrangian warps (896 threads launched at 72 registers each, re-split with setmaxnreg to 80 / 56:
+// nothing spills).
 #ifndef GP_GAS_FY
 #define GP_GAS_FY 16
 #define GP_GAS_NDW 12
 #endif
 #ifndef GP_GAS_REG_E
-#define GP_GAS_REG_E 72
-#define GP_GAS_REG_D 64
+#define GP_GAS_REG_E 80
+#define GP_GAS_REG_D 56
 #endif
 #ifndef GP_GAS_NS
 #define GP_GAS_NS 6

@@ -58,6 +58,14 @@ constexpr int DROWS = TYO / NDW;          // output rows per Lagrangian warp
 #ifndef GP_NS
 #define GP_NS 4
 #endif
+// GP_OVERDET (contexts created with GP_OD): the kernels also carry the overdetermined system (PAPER.md:41 4th equation): one more gas field
+// (rho*eps, paired with the energy), six more collisionless fields (Pi_ij); pressure and dispersion tensor of the
+// face solvers come from the carried fields; kappa and the energy balance (G15) sit in
+// the epilogue of the Lagrangian stage.
+#ifndef GP_OVERDET
+#define GP_OVERDET 0
+#endif
+constexpr bool OD = GP_OVERDET != 0;
 constexpr int NS = GP_NS;                 // slots of the U* ring: planes j-2, j-1, j of the Lagrangian warps and NS - 3 ahead
 constexpr int NPHI = NS + 2;              // slots of the Phi ring
 constexpr int NTZ = NS - 2;               // buffers of the z-averaged face-velocity plane
@@ -112,28 +120,28 @@ __device__ __forceinline__ int map_safe(int i, int n, int bc) {
 // formulas fold into the flux coefficients tau/(2h), tau/(4h) (exact power-of-two scalings).
 //
 // PAPER.md:112, 114 with Z = sqrt(rl rr gamma (pl+pr)/(rl+rr)) = num*r, 1/Z = den*r, r = rsqrt(num*den).
-// Out: P2 = 2P, PV4 = 4 P V.
+// Out: P2 = 2P, PV4 = 4 P V, V2 = 2V.
 __device__ __forceinline__ void gas_face(double gamma, double rl, double vl, double pl, double rr, double vr, double pr,
-                                         double& P2, double& PV4) {
+                                         double& P2, double& PV4, double& V2) {
     const double ps = pl + pr;
     const double num = rl * rr * (gamma * ps), den = rl + rr;
     const double r = frsqrt(num * den);
     const double Z = num * r, iZ = den * r;
-    const double V2 = fma(pl - pr, iZ, vl + vr);
+    V2 = fma(pl - pr, iZ, vl + vr);
     P2 = fma(vl - vr, Z, ps);
     PV4 = P2 * V2;
 }
 
 // PAPER.md:170-178 for a face normal to axis D, bracketed parameters averaged (PAPER.md:180,
 // reading G7).  In: n, u[3], Pd[3] = Pi_{xD}, Pi_{yD}, Pi_{zD} of both sides.
-// Out: Ps2[3] = 2 Pi*_{.D} (momentum flux) and EF4[6] = 4 (Pi*_{jD} u*_i + Pi*_{iD} u*_j) for
-// (i,j) = xx xy xz yy yz zz (flux of nE_ij).
+// Out: Ps2[3] = 2 Pi*_{.D} (momentum flux), EF4[6] = 4 (Pi*_{jD} u*_i + Pi*_{iD} u*_j) for
+// (i,j) = xx xy xz yy yz zz (flux of nE_ij) and us2[3] = 2 u* (PAPER.md:170-172).
 // With q = nl nr, s = nl+nr, A = Pl+Pr (= 2a):  [rho] a = q A / s,  Z1 = sqrt([rho] a) = q A r,
 // 1/Z1 = s r, 1/a = 2 q s r^2, where r = rsqrt(q A s).
 template <int D>
 __device__ __forceinline__ void bme_face(double nl, const double ul[3], const double Pl[3],
                                          double nr, const double ur[3], const double Pr[3],
-                                         double Ps2[3], double EF4[6]) {
+                                         double Ps2[3], double EF4[6], double us2[3]) {
     const double s3 = 1.7320508075688772935, is3 = 0.57735026918962576451;
     const double q = nl * nr, s = nl + nr;
     const double A = Pl[D] + Pr[D];
@@ -143,7 +151,6 @@ __device__ __forceinline__ void bme_face(double nl, const double ul[3], const do
     const double ia = (q * s) * (2.0 * r * r);
     const double Z3 = s3 * Z1, iZ3 = is3 * iZ1;
     const double DP = Pl[D] - Pr[D], DU = ul[D] - ur[D];
-    double us2[3];
     us2[D] = fma(DP, iZ3, ul[D] + ur[D]);
     Ps2[D] = fma(DU, Z3, A);
     // b ku = (B/2) (1-sqrt3) (DP/2) / (a Z3) and doubled: B * [(1-sqrt3)/2 * ia * iZ3 * DP]
@@ -350,6 +357,8 @@ struct FusedArgs {
     int* flag;
     const double* src_in;     // gas kernel only: density n of the new collisionless state, or null
     double* src_out;          // ... and where to write the Poisson source rho + n of the new state, or null
+    int balance;              // GP_OD: apply the energy balance (G15) to the new state
+    double* kappa;            // GP_OD: += sum over cells of this component's kappa integrand, before the balance
 };
 
 // Small per-block tables (shared memory, written once by thread 0).
@@ -436,30 +445,36 @@ __device__ __forceinline__ void stage_phi(const FusedArgs<NF>& a, const BlockTab
 }
 
 // block maximum of the signal speed -> one atomicMax of the bit pattern (speeds are >= 0)
+// (GP_OD: and the block's sum of the kappa integrand -> one atomicAdd)
 __device__ __forceinline__ void block_max_commit(double smax, int bad, unsigned long long* smax_bits, int* flag,
-                                                 double* scratch) {
+                                                 double* scratch, double kap = 0.0, double* kappa = nullptr) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
         bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+        if (OD) kap += __shfl_xor_sync(0xffffffffu, kap, o);
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     constexpr int NW = NT / 32;
     int* sbad = (int*)(scratch + NW);
-    if (lane == 0) { scratch[warp] = smax; sbad[warp] = bad; }
+    double* skap = scratch + 2 * NW;
+    if (lane == 0) { scratch[warp] = smax; sbad[warp] = bad; if (OD) skap[warp] = kap; }
     __syncthreads();
     if (warp == 0) {
         smax = lane < NW ? scratch[lane] : 0.0;
         bad = lane < NW ? sbad[lane] : 0;
+        kap = (OD && lane < NW) ? skap[lane] : 0.0;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
             bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+            if (OD) kap += __shfl_xor_sync(0xffffffffu, kap, o);
         }
         if (lane == 0) {
             atomicMax(smax_bits, (unsigned long long)__double_as_longlong(smax));
             if (bad) atomicOr(flag, 1);
+            if (OD && kappa) atomicAdd(kappa, kap);
         }
     }
 }
@@ -504,7 +519,7 @@ __device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b, const Bloc
 // Per-thread state of a Lagrangian thread: DROWS output cells (rows 2 + w + NDW q of the footprint, column lane).
 struct LagRows {
     double Sz_prev[DROWS], wzp_prev[DROWS], pre[DROWS];
-    double smax;
+    double smax, kap;
     int bad;
 };
 
@@ -532,7 +547,7 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
         row_off[q] = (size_t)xv + (size_t)g.nx * yv;
         L.Sz_prev[q] = L.wzp_prev[q] = L.pre[q] = 0.0;
     }
-    L.smax = 0.0; L.bad = 0;
+    L.smax = 0.0; L.kap = 0.0; L.bad = 0;
     // prologue: Phi(z0-2 .. z0) for the first B and C, then the bundles (U(k+1), Phi(k+2)) of the first NS - 2 planes
     // k = z0-1 ... into ring slots 0 ...; E(k) consumes bundle k
     if (bulk && dtid == 0) mbar_arrive_expect_tx(&T->pro, 3 * PBYTES);
@@ -617,7 +632,7 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
                 if (lag_needed(lc.ym, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(r0, t - FX, lc.ym, out);
                 if (lag_needed(lc.yp, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(r0, t + FX, lc.yp, out);
                 if (lag_needed(lc.zp, lane_out)) lagrange_add<TR::NP2, TR::LAST1, false>(rs, t, lc.zp, out);
-                if (is_out) TR::emit(a, off, out, pre, L.smax, L.bad);
+                if (is_out) TR::emit(a, off, out, pre, L.smax, L.bad, L.kap);
             }
         }
     }
@@ -629,27 +644,53 @@ __device__ __forceinline__ void lag_warps(const FusedArgs<NF>& a, BlockTab* T, c
 // Shared planes (of PL doubles): (rho,p) pair 2, vx 1, vy 1, Phi ring 8, y-flux (P,PV) pair 2,
 // U* ring 4 x (2 pair planes + 1 plain) = 20, z-averaged (w*_x,w*_y) pair 2 x 2 = 4  ->  38 planes.
 // =================================================================================================
+// GP_OD: one more field, rho*eps, paired with the energy: (rho E, rho eps) in HBM and in the ring; the y-flux exchange
+// carries 2V as a third value.
+constexpr int NFG = NGAS + (OD ? NODG : 0);
+constexpr int IEPS = OD ? NGAS : 0;       // rho*eps among the fields (only used under GP_OD; in range either way)
 struct GasTraits {
-    static constexpr int NPAIR = 2, NP2 = 0;
-    static constexpr bool LAST1 = true;
-    static constexpr int SLOT = 2 * PP + PL;
-    static constexpr int PLANES = 2 + 1 + 1 + NPHI + 2 + NS * 5 + 2 * NTZ;
+    static constexpr int NPAIR = OD ? 3 : 2, NP2 = OD ? 1 : 0;
+    static constexpr bool LAST1 = !OD;
+    static constexpr int SLOT = OD ? 3 * PP : 2 * PP + PL;
+    static constexpr int PLANES = 2 + 1 + 1 + NPHI + (OD ? 3 : 2) + NS * (OD ? 6 : 5) + 2 * NTZ;
     // density of the other component for the Poisson source, asked for one plane before it is used
-    __device__ static __forceinline__ double early(const FusedArgs<NGAS>& a, size_t off, bool is_out) {
+    __device__ static __forceinline__ double early(const FusedArgs<NFG>& a, size_t off, bool is_out) {
         return (a.src_in && is_out) ? a.src_in[BSTR * off] : 0.0;
     }
-    __device__ static __forceinline__ void emit(const FusedArgs<NGAS>& a, size_t off, const double out[NGAS], double n_other, double& smax,
-                                                int& bad) {
-#pragma unroll
-        for (int P = 0; P < NGASP / 2; ++P)
-            *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
-        a.Un[4][off] = out[4];
-        if (a.src_out) a.src_out[off] = out[0] + n_other;   // PAPER.md:186
-        // CFL of the new state (reading G4)
+    __device__ static __forceinline__ void emit(const FusedArgs<NFG>& a, size_t off, double out[NFG], double n_other, double& smax,
+                                                int& bad, double& kap) {
         const double gm1 = a.gamma - 1.0;
         const double irn = frcp(out[0]);
-        const double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
-        const double pn = gm1 * (out[4] - 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz)));
+        double ux = out[1] * irn, uy = out[2] * irn, uz = out[3] * irn;
+        double kin = 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz));
+        if (OD) {
+            // correctness check of the state as the two stages left it, then the energy balance (G15)
+            const double e_tot = out[4] - kin;            // rho eps as the total energy implies it
+            kap += fabs(e_tot - out[IEPS]);
+            if (a.balance) {
+                if (e_tot > 0.0) {
+                    out[IEPS] = e_tot;
+                } else {                                  // gas-vacuum border: the carried internal energy wins
+                    const double kin_new = out[4] - out[IEPS];
+                    if (kin_new > 0.0 && kin > 0.0) {
+                        const double sc = sqrt(kin_new / kin);
+                        out[1] *= sc; out[2] *= sc; out[3] *= sc;
+                        ux *= sc; uy *= sc; uz *= sc;
+                        kin = 0.5 * fma(out[1], ux, fma(out[2], uy, out[3] * uz));
+                    } else {
+                        out[1] = out[2] = out[3] = 0.0; ux = uy = uz = 0.0; kin = 0.0;
+                        out[4] = out[IEPS];
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int P = 0; P < NPAIR; ++P)
+            *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
+        if (LAST1) a.Un[4][off] = out[4];
+        if (a.src_out) a.src_out[off] = out[0] + n_other;   // PAPER.md:186
+        // CFL of the new state (reading G4)
+        const double pn = gm1 * (out[4] - kin);
         const double c2 = a.gamma * pn * irn;
         const double sp = fmax(fmax(fabs(ux), fabs(uy)), fabs(uz)) + c2 * frsqrt(c2);
         if (!(out[0] > 0.0) || !(pn > 0.0) || !(sp <= 1.7976931348623157e308)) bad = 1;
@@ -660,14 +701,15 @@ struct GasTraits {
 struct GasCarry {
     double rho, ir, vx, vy, vz, p;        // primitives of the current plane j (own cell)
     double amx, amy, amz, aE;             // U*(j) under construction
+    double eps, adv;                      // GP_OD: rho*eps of plane j; 2 x (sum of V_hi - V_lo over the faces done so far)
 };
 
 struct GasShared {
-    double *rp, *vx, *vy, *phi, *fy, *ring, *tz;
+    double *rp, *vx, *vy, *phi, *fy, *fyv, *ring, *tz;
 };
 
 template <bool ST>
-__device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, const Blk& b, const Foot& f, const GasShared& S,
+__device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, const Blk& b, const Foot& f, const GasShared& S,
                                          GasCarry& c, int j, double tau, double th, double inv2h) {
     const Geo& g = a.g;
     const int t = f.t;
@@ -683,17 +725,18 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
 
     // B: x and y faces of plane j, each computed once (hi face per thread), in one basic block so
     // that the two solvers interleave
-    double Pyh = 0.0, PVyh = 0.0, gy = 0.0;
+    double Pyh = 0.0, PVyh = 0.0, Vyh = 0.0, gy = 0.0;
     if (f.star_row) {
         const int tr = f.tx < FX - 1 ? t + 1 : t;
         const double2 ry = lds2(S.rp + 2 * (t + FX)), rx = lds2(S.rp + 2 * tr);
         const double vyr = S.vy[t + FX], vxr = S.vx[tr];
         const double phe = ph0[tr], phn = ph0[t + FX];
         const double phw = ph0[f.tx > 0 ? t - 1 : t], phs = ph0[t - FX];
-        double Pxh, PVxh;
-        gas_face(gamma, c.rho, c.vy, c.p, ry.x, vyr, ry.y, Pyh, PVyh);
-        gas_face(gamma, c.rho, c.vx, c.p, rx.x, vxr, rx.y, Pxh, PVxh);
+        double Pxh, PVxh, Vxh;
+        gas_face(gamma, c.rho, c.vy, c.p, ry.x, vyr, ry.y, Pyh, PVyh, Vyh);
+        gas_face(gamma, c.rho, c.vx, c.p, rx.x, vxr, rx.y, Pxh, PVxh, Vxh);
         sts2(S.fy + 2 * t, Pyh, PVyh);
+        if (OD) { S.fyv[t] = Vyh; c.adv += Vxh - __shfl_up_sync(0xffffffffu, Vxh, 1); }
         const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1);
         const double PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
         const double gx = (phe - phw) * inv2h;
@@ -705,8 +748,9 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     } else if (f.ty == 0) {
         // the lowest halo row only supplies the y face between itself and row 1; the top halo row supplies nothing
         const double2 ry = lds2(S.rp + 2 * (t + FX));
-        gas_face(gamma, c.rho, c.vy, c.p, ry.x, S.vy[t + FX], ry.y, Pyh, PVyh);
+        gas_face(gamma, c.rho, c.vy, c.p, ry.x, S.vy[t + FX], ry.y, Pyh, PVyh, Vyh);
         sts2(S.fy + 2 * t, Pyh, PVyh);
+        if (OD) S.fyv[t] = Vyh;
     }
     row_arrive_at<OY_OWN>(f.rowbar);                                  // y fluxes of this row are written
     if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);       // ... and those of the row below
@@ -718,6 +762,7 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
         const double my = c.rho * c.vy;
         c.amy = c.amy - th2 * (Pyh - lo.x) - trg;
         c.aE = c.aE - th4 * (PVyh - lo.y) - fma(-0.5 * tau, trg, tau * my) * gy;
+        if (OD) c.adv += Vyh - S.fyv[t - FX];
     }
 
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
@@ -726,18 +771,24 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     const unsigned slotbar = f.tabbar + 8 * rslot(it);
     mbar_wait_at<0>(slotbar, rpar(it));
     const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t);
-    const double rho_n = s0.x, mx_n = s0.y, my_n = s1.x, mz_n = s1.y, E_n = rs[2 * PP + t];
+    double E_n, eps_n = 0.0;
+    if (OD) { const double2 s2 = lds2(rs + 2 * PP + 2 * t); E_n = s2.x; eps_n = s2.y; }
+    else E_n = rs[2 * PP + t];
+    const double rho_n = s0.x, mx_n = s0.y, my_n = s1.x, mz_n = s1.y;
     const double ir_n = frcp(rho_n);
     const double vx_n = mx_n * ir_n, vy_n = my_n * ir_n, vz_n = mz_n * ir_n;
-    const double p_n = gm1 * (E_n - 0.5 * fma(mx_n, vx_n, fma(my_n, vy_n, mz_n * vz_n)));
-    double Pz = 0.0, PVz = 0.0;
+    // GP_OD: the pressure comes from the carried internal energy (4th equation)
+    const double p_n = OD ? gm1 * eps_n : gm1 * (E_n - 0.5 * fma(mx_n, vx_n, fma(my_n, vy_n, mz_n * vz_n)));
+    double Pz = 0.0, PVz = 0.0, Vz = 0.0;
     if (f.star_row) {
-        gas_face(gamma, c.rho, c.vz, c.p, rho_n, vz_n, p_n, Pz, PVz);
-        double wx, wy, wz, Es, dens;
+        gas_face(gamma, c.rho, c.vz, c.p, rho_n, vz_n, p_n, Pz, PVz, Vz);
+        double wx, wy, wz, Es, dens, epss = 0.0;
         if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
             const double* rq = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
             const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
-            dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y; Es = rq[2 * PP + t];
+            dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y;
+            if (OD) { const double2 q2 = lds2(rq + 2 * PP + 2 * t); Es = q2.x; epss = q2.y; }
+            else Es = rq[2 * PP + t];
         } else {
             const double gz = (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h;
             const double trg = tau * c.rho * gz;
@@ -745,11 +796,15 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
             const double mzs = c.amz - th2 * Pz - trg;
             Es = c.aE - th4 * PVz - fma(-0.5 * tau, trg, tau * mz) * gz;
             dens = c.rho; wx = c.amx * c.ir; wy = c.amy * c.ir; wz = mzs * c.ir;
+            // (rho eps)* = rho eps - tau (gamma-1) rho eps div V, V the face values of PAPER.md:112
+            if (OD) epss = fma(-(th2 * gm1) * c.eps, c.adv + Vz, c.eps);
         }
-        sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy); rs[2 * PP + t] = Es;
+        sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy);
+        if (OD) sts2(rs + 2 * PP + 2 * t, Es, epss); else rs[2 * PP + t] = Es;
         if (bot_dup) {                        // outflow: U*(-1) := U*(0)
             double* rg = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
-            sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy); rg[2 * PP + t] = Es;
+            sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy);
+            if (OD) sts2(rg + 2 * PP + 2 * t, Es, epss); else rg[2 * PP + t] = Es;
         }
         if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
             const double2 wm = lds2(S.ring + rslot(it + NS - 2) * GasTraits::SLOT + PP + 2 * t);
@@ -760,20 +815,23 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
     sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
     c.amx = mx_n; c.amy = my_n; c.amz = fma(th2, Pz, mz_n); c.aE = fma(th4, PVz, E_n);
     c.rho = rho_n; c.ir = ir_n; c.vx = vx_n; c.vy = vy_n; c.vz = vz_n; c.p = p_n;
+    if (OD) { c.eps = eps_n; c.adv = -Vz; }
     row_arrive_at<OP_OWN>(f.rowbar);                                  // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
         if (f.fix) {
 #pragma unroll
-            for (int P = 0; P < 2; ++P) {
+            for (int P = 0; P < GasTraits::NPAIR; ++P) {
                 const double2 v = lds2(rs + P * PP + 2 * f.fix_src);
                 sts2(rs + P * PP + 2 * t, v.x, v.y);
                 if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + P * PP + 2 * t, v.x, v.y);
             }
-            const double e = rs[2 * PP + f.fix_src];
-            rs[2 * PP + t] = e;
-            if (bot_dup) S.ring[rslot(it + NS - 1) * GasTraits::SLOT + 2 * PP + t] = e;
+            if (GasTraits::LAST1) {
+                const double e = rs[2 * PP + f.fix_src];
+                rs[2 * PP + t] = e;
+                if (bot_dup) S.ring[rslot(it + NS - 1) * GasTraits::SLOT + 2 * PP + t] = e;
+            }
             const double2 v = lds2(S.tz + (it % NTZ) * PP + 2 * f.fix_src);
             sts2(S.tz + (it % NTZ) * PP + 2 * t, v.x, v.y);
         }
@@ -784,13 +842,14 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NGAS>& a, BlockTab* T, 
 }
 
 __global__ void __launch_bounds__(NT, 1)
-k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
+k_fused_gas(const __grid_constant__ FusedArgs<NFG> a) {
     extern __shared__ __align__(128) unsigned char smraw[];
     BlockTab* T = reinterpret_cast<BlockTab*>(smraw);
     double* sm = reinterpret_cast<double*>(smraw + sizeof(BlockTab));
     GasShared S;
     S.rp = sm; S.vx = sm + 2 * PL; S.vy = sm + 3 * PL; S.phi = sm + 4 * PL; S.fy = S.phi + NPHI * PL;
-    S.ring = S.fy + 2 * PL; S.tz = S.ring + NS * GasTraits::SLOT;
+    S.fyv = S.fy + 2 * PL;
+    S.ring = S.fyv + (OD ? PL : 0); S.tz = S.ring + NS * GasTraits::SLOT;
 
     const Geo& g = a.g;
     const Blk b = make_blk(g, a.zchunk);
@@ -808,7 +867,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
     const double tau = a.dt_ptr ? *a.dt_ptr : a.dt_val;
     const double th = tau / a.h, inv2h = 0.5 / a.h, gm1 = a.gamma - 1.0;
 
-    double smax = 0.0;
+    double smax = 0.0, kap = 0.0;
     int bad = 0;
     if (threadIdx.x >= NTE) {
 #if GP_REG_D
@@ -816,7 +875,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
 #endif
         LagRows L;
         lag_warps<GasTraits>(a, T, b, S.ring, S.tz, S.phi, th, L);
-        smax = L.smax; bad = L.bad;
+        smax = L.smax; bad = L.bad; kap = L.kap;
     } else {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
@@ -827,20 +886,23 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
         {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
             int zm = map_safe(b.z0 - 2, g.nz, g.bcz);
             size_t off = f.base + (size_t)zm * f.nxny;
-            double rho = a.U[0][BSTR * off], mx = a.U[1][BSTR * off], my = a.U[2][BSTR * off], mz = a.U[3][BSTR * off], E = a.U[4][off];
+            constexpr int ES = OD ? BSTR : 1;        // the energy is paired with rho*eps under GP_OD
+            double rho = a.U[0][BSTR * off], mx = a.U[1][BSTR * off], my = a.U[2][BSTR * off], mz = a.U[3][BSTR * off], E = a.U[4][ES * off];
             double ir = frcp(rho);
             const double vz_a = mz * ir;
             // same expression as the main loop, so that a 1-D problem stays bitwise 1-D across the chunk edge
-            const double p_a = gm1 * (E - 0.5 * fma(mx, mx * ir, fma(my, my * ir, mz * vz_a)));
+            const double p_a = OD ? gm1 * a.U[IEPS][BSTR * off] : gm1 * (E - 0.5 * fma(mx, mx * ir, fma(my, my * ir, mz * vz_a)));
             const double rho_a = rho;
             zm = map_safe(b.z0 - 1, g.nz, g.bcz);
             off = f.base + (size_t)zm * f.nxny;
-            rho = a.U[0][BSTR * off]; mx = a.U[1][BSTR * off]; my = a.U[2][BSTR * off]; mz = a.U[3][BSTR * off]; E = a.U[4][off];
+            rho = a.U[0][BSTR * off]; mx = a.U[1][BSTR * off]; my = a.U[2][BSTR * off]; mz = a.U[3][BSTR * off]; E = a.U[4][ES * off];
             ir = frcp(rho);
             c.rho = rho; c.ir = ir; c.vx = mx * ir; c.vy = my * ir; c.vz = mz * ir;
-            c.p = gm1 * (E - 0.5 * fma(mx, c.vx, fma(my, c.vy, mz * c.vz)));
-            double Pz, PVz;
-            gas_face(a.gamma, rho_a, vz_a, p_a, c.rho, c.vz, c.p, Pz, PVz);
+            c.eps = OD ? a.U[IEPS][BSTR * off] : 0.0;
+            c.p = OD ? gm1 * c.eps : gm1 * (E - 0.5 * fma(mx, c.vx, fma(my, c.vy, mz * c.vz)));
+            double Pz, PVz, Vz;
+            gas_face(a.gamma, rho_a, vz_a, p_a, c.rho, c.vz, c.p, Pz, PVz, Vz);
+            c.adv = -Vz;
             c.amx = mx; c.amy = my; c.amz = fma(0.5 * th, Pz, mz); c.aE = fma(0.25 * th, PVz, E);
             sts2(S.rp + 2 * t, c.rho, c.p); S.vx[t] = c.vx; S.vy[t] = c.vy;
         }
@@ -852,7 +914,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
         for (; j <= b.z1 - 1; ++j) gas_iter<true>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1; ++j) gas_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
     }
-    block_max_commit(smax, bad, a.smax_bits, a.flag, S.rp);
+    block_max_commit(smax, bad, a.smax_bits, a.flag, S.rp, kap, a.kappa);
 }
 
 #endif  // GP_FUSED_GAS
@@ -864,18 +926,50 @@ k_fused_gas(const __grid_constant__ FusedArgs<NGAS> a) {
 // Phi ring 8, y-flux (Ps0,Ps1) (Ps2,EF0) (EF1,EF2) (EF3,EF4) pairs 8 + EF5 1, U* ring 4 x 5 pair planes = 40,
 // z-averaged (w*_x,w*_y) pair 2 x 2 = 4  ->  70 planes (210 KB at FY = 12).
 // =================================================================================================
+// GP_OD: six more fields, Pi_ij, as three more pairs (Pi_xx,Pi_xy) (Pi_xz,Pi_yy) (Pi_yz,Pi_zz) in HBM and in the
+// ring; the y-flux exchange carries 2u* as three more values: (EF5,us0) (us1,us2).
+constexpr int NFB = NBME + (OD ? NODB : 0);
+constexpr int PI0 = OD ? NBME : 0;        // first carried Pi_ij among the fields (only used under GP_OD; in range either way)
+__device__ __forceinline__ constexpr int symi(int i, int j) {      // (i,j) -> index in xx xy xz yy yz zz
+    return i == 0 ? j : (j == 0 ? i : (i == 1 ? (j == 1 ? 3 : 4) : (j == 1 ? 4 : 5)));
+}
 struct BmeTraits {
-    static constexpr int NPAIR = 5, NP2 = 3;
+    static constexpr int NPAIR = OD ? 8 : 5, NP2 = NPAIR - 2;
     static constexpr bool LAST1 = false;
-    static constexpr int SLOT = 5 * PP;
-    static constexpr int PLANES = 9 + NPHI + 9 + NS * 10 + 2 * NTZ;
-    __device__ static __forceinline__ double early(const FusedArgs<NBME>&, size_t, bool) { return 0.0; }
-    __device__ static __forceinline__ void emit(const FusedArgs<NBME>& a, size_t off, const double out[NBME], double, double& smax, int& bad) {
+    static constexpr int SLOT = NPAIR * PP;
+    static constexpr int NFY = OD ? 12 : 9;      // planes of the y-flux exchange
+    static constexpr int PLANES = 9 + NPHI + NFY + NS * 2 * NPAIR + 2 * NTZ;
+    __device__ static __forceinline__ double early(const FusedArgs<NFB>&, size_t, bool) { return 0.0; }
+    __device__ static __forceinline__ void emit(const FusedArgs<NFB>& a, size_t off, double out[NFB], double, double& smax, int& bad,
+                                                double& kap) {
+        const double inn = frcp(out[0]);
+        if (OD) {
+            // correctness check of the state as the two stages left it, then the energy balance (G15)
+            const double u[3] = {out[1] * inn, out[2] * inn, out[3] * inn};
+            double Pc[6];                                 // Pi_ij as the total-energy tensor implies it
 #pragma unroll
-        for (int P = 0; P < NBME / 2; ++P)
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+                for (int j = i; j < 3; ++j) {
+                    Pc[symi(i, j)] = fma(-out[1 + i], u[j], out[4 + symi(i, j)]);
+                    kap += fabs(Pc[symi(i, j)] - out[PI0 + symi(i, j)]);
+                }
+            if (a.balance) {
+                if (Pc[0] > 0.0 && Pc[3] > 0.0 && Pc[5] > 0.0) {
+#pragma unroll
+                    for (int q = 0; q < 6; ++q) out[PI0 + q] = Pc[q];
+                } else {                                  // the carried tensor wins
+#pragma unroll
+                    for (int i = 0; i < 3; ++i)
+#pragma unroll
+                        for (int j = i; j < 3; ++j) out[4 + symi(i, j)] = fma(out[1 + i], u[j], out[PI0 + symi(i, j)]);
+                }
+            }
+        }
+#pragma unroll
+        for (int P = 0; P < NPAIR; ++P)
             *reinterpret_cast<double2*>(a.Un[2 * P] + BSTR * off) = make_double2(out[2 * P], out[2 * P + 1]);
         // CFL of the new state (reading G4): |u_d| + sqrt(3 Pi_dd / n)
-        const double inn = frcp(out[0]);
         const int dd[3] = {4, 7, 9};
         if (!(out[0] > 0.0)) bad = 1;
 #pragma unroll
@@ -893,14 +987,35 @@ struct BmeTraits {
 struct BmeCarry {
     double n, in, u[3], Pi[6];            // primitives of the current plane j (own cell)
     double acc[9];                        // U*(j) under construction: nu (3), nE (6)
+    double accP[6];                       // GP_OD: Pi*(j) under construction
 };
+
+// y-flux exchange of one cell: Py (3), EFy (6) and, under GP_OD, 2u* (3)
+__device__ __forceinline__ void fy_store(double* fy, int t, const double Py[3], const double EFy[6], const double usy[3]) {
+    sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
+    sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
+    if (OD) { sts2(fy + 4 * PP + 2 * t, EFy[5], usy[0]); sts2(fy + 5 * PP + 2 * t, usy[1], usy[2]); }
+    else fy[4 * PP + t] = EFy[5];
+}
+
+// GP_OD, PAPER.md:65 without advection: Pi*_ab -= (tau/h) [Pi_bk du_a + Pi_ak du_b] for the faces normal to axis K,
+// du2 = 2 x (u*_hi - u*_lo) of that axis, Pi the carried tensor of the cell at time n; sg = -1 for the hi - lo
+// difference, +1 when only the lo face is entered (with du2 = 2 u*_lo)
+template <int K>
+__device__ __forceinline__ void pi_source(double accP[6], const double Pi[6], const double du2[3], double sth2) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = i; j < 3; ++j)
+            accP[symi(i, j)] = fma(sth2, fma(Pi[symi(j, K)], du2[i], Pi[symi(i, K)] * du2[j]), accP[symi(i, j)]);
+}
 
 struct BmeShared {
     double *nu, *uu, *px, *py, *pxy, *phi, *fy, *ring, *tz;
 };
 
 template <bool ST>
-__device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, const Blk& b, const Foot& f, const BmeShared& S,
+__device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, const Blk& b, const Foot& f, const BmeShared& S,
                                          BmeCarry& c, int j, double tau, double th, double inv2h) {
     const Geo& g = a.g;
     const int t = f.t;
@@ -915,7 +1030,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
 
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
     // dependent chains interleave
-    double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, usy[3] = {0.0, 0.0, 0.0};
     double gx = 0.0, gy = 0.0;
     if (f.star_row) {
         const int tn = t + FX, te = f.tx < FX - 1 ? t + 1 : t;
@@ -925,13 +1040,16 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         const double ury[3] = {y0.y, y1.x, y1.y}, urx[3] = {x0.y, x1.x, x1.y};
         const double Ply[3] = {c.Pi[1], c.Pi[3], c.Pi[4]}, Plx[3] = {c.Pi[0], c.Pi[1], c.Pi[2]};
         const double Pry[3] = {pxy_n, y2.x, y2.y}, Prx[3] = {x2.x, pxy_e, x2.y};
-        double Px[3], EFx[6];
-        bme_face<1>(c.n, c.u, Ply, y0.x, ury, Pry, Py, EFy);
-        bme_face<0>(c.n, c.u, Plx, x0.x, urx, Prx, Px, EFx);
-        double* fy = S.fy;
-        sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
-        sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
-        fy[4 * PP + t] = EFy[5];
+        double Px[3], EFx[6], usx[3];
+        bme_face<1>(c.n, c.u, Ply, y0.x, ury, Pry, Py, EFy, usy);
+        bme_face<0>(c.n, c.u, Plx, x0.x, urx, Prx, Px, EFx, usx);
+        fy_store(S.fy, t, Py, EFy, usy);
+        if (OD) {
+            double du2[3];
+#pragma unroll
+            for (int q = 0; q < 3; ++q) du2[q] = usx[q] - __shfl_up_sync(0xffffffffu, usx[q], 1);
+            pi_source<0>(c.accP, c.Pi, du2, -th2);
+        }
 #pragma unroll
         for (int q = 0; q < 3; ++q) c.acc[q] -= th2 * (Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1));
 #pragma unroll
@@ -945,11 +1063,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
         const double ury[3] = {y0.y, y1.x, y1.y};
         const double Ply[3] = {c.Pi[1], c.Pi[3], c.Pi[4]};
         const double Pry[3] = {S.pxy[tn], y2.x, y2.y};
-        bme_face<1>(c.n, c.u, Ply, y0.x, ury, Pry, Py, EFy);
-        double* fy = S.fy;
-        sts2(fy + 2 * t, Py[0], Py[1]); sts2(fy + PP + 2 * t, Py[2], EFy[0]);
-        sts2(fy + 2 * PP + 2 * t, EFy[1], EFy[2]); sts2(fy + 3 * PP + 2 * t, EFy[3], EFy[4]);
-        fy[4 * PP + t] = EFy[5];
+        bme_face<1>(c.n, c.u, Ply, y0.x, ury, Pry, Py, EFy, usy);
+        fy_store(S.fy, t, Py, EFy, usy);
     }
     row_arrive_at<OY_OWN>(f.rowbar);                                  // y fluxes of this row are written
     if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);       // ... and those of the row below
@@ -958,7 +1073,15 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     if (f.star_row) {
         const double* fy = S.fy + 2 * (t - FX);
         const double2 l0 = lds2(fy), l1 = lds2(fy + PP), l2 = lds2(fy + 2 * PP), l3 = lds2(fy + 3 * PP);
-        const double l4 = S.fy[4 * PP + t - FX];
+        double l4;
+        if (OD) {
+            const double2 m4 = lds2(fy + 4 * PP), m5 = lds2(fy + 5 * PP);
+            l4 = m4.x;
+            const double du2[3] = {usy[0] - m4.y, usy[1] - m5.x, usy[2] - m5.y};
+            pi_source<1>(c.accP, c.Pi, du2, -th2);
+        } else {
+            l4 = S.fy[4 * PP + t - FX];
+        }
         c.acc[0] -= th2 * (Py[0] - l0.x); c.acc[1] -= th2 * (Py[1] - l0.y); c.acc[2] -= th2 * (Py[2] - l1.x);
         c.acc[3] -= th4 * (EFy[0] - l1.y); c.acc[4] -= th4 * (EFy[1] - l2.x); c.acc[5] -= th4 * (EFy[2] - l2.y);
         c.acc[6] -= th4 * (EFy[3] - l3.x); c.acc[7] -= th4 * (EFy[4] - l3.y); c.acc[8] -= th4 * (EFy[5] - l4);
@@ -983,44 +1106,62 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     double* rs = S.ring + rslot(it) * BmeTraits::SLOT;
     const unsigned slotbar = f.tabbar + 8 * rslot(it);
     mbar_wait_at<0>(slotbar, rpar(it));
-    double Un[NBME];
+    double Un[NFB];
     {
-        const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t), s2 = lds2(rs + 2 * PP + 2 * t),
-                      s3 = lds2(rs + 3 * PP + 2 * t), s4 = lds2(rs + 4 * PP + 2 * t);
-        Un[0] = s0.x; Un[1] = s0.y; Un[2] = s1.x; Un[3] = s1.y; Un[4] = s2.x; Un[5] = s2.y;
-        Un[6] = s3.x; Un[7] = s3.y; Un[8] = s4.x; Un[9] = s4.y;
+        const double2 s0 = lds2(rs + 2 * t), s1 = lds2(rs + PP + 2 * t);
+        Un[0] = s0.x; Un[1] = s0.y; Un[2] = s1.x; Un[3] = s1.y;
+#pragma unroll
+        for (int P = 2; P < BmeTraits::NPAIR; ++P) {
+            const double2 sp = lds2(rs + P * PP + 2 * t);
+            Un[2 * P] = sp.x; Un[2 * P + 1] = sp.y;
+        }
     }
     const double n_n = Un[0];
     const double in_n = frcp(n_n);
     const double u_n[3] = {Un[1] * in_n, Un[2] * in_n, Un[3] * in_n};
     double Pi_n[6];
-    Pi_n[0] = fma(-Un[1], u_n[0], Un[4]); Pi_n[1] = fma(-Un[1], u_n[1], Un[5]); Pi_n[2] = fma(-Un[1], u_n[2], Un[6]);
-    Pi_n[3] = fma(-Un[2], u_n[1], Un[7]); Pi_n[4] = fma(-Un[2], u_n[2], Un[8]); Pi_n[5] = fma(-Un[3], u_n[2], Un[9]);
-    double Pz[3] = {0.0, 0.0, 0.0}, EFz[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (OD) {        // the dispersion tensor as carried
+#pragma unroll
+        for (int q = 0; q < 6; ++q) Pi_n[q] = Un[PI0 + q];
+    } else {
+        Pi_n[0] = fma(-Un[1], u_n[0], Un[4]); Pi_n[1] = fma(-Un[1], u_n[1], Un[5]); Pi_n[2] = fma(-Un[1], u_n[2], Un[6]);
+        Pi_n[3] = fma(-Un[2], u_n[1], Un[7]); Pi_n[4] = fma(-Un[2], u_n[2], Un[8]); Pi_n[5] = fma(-Un[3], u_n[2], Un[9]);
+    }
+    double Pz[3] = {0.0, 0.0, 0.0}, EFz[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, usz[3] = {0.0, 0.0, 0.0};
     if (f.star_row) {
         const double Pl[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
         const double Pr[3] = {Pi_n[2], Pi_n[4], Pi_n[5]};
-        bme_face<2>(c.n, c.u, Pl, n_n, u_n, Pr, Pz, EFz);
-        double o[NBME];      // n, w (3), nE (6)
+        bme_face<2>(c.n, c.u, Pl, n_n, u_n, Pr, Pz, EFz, usz);
+        double o[NFB];      // n, w (3), nE (6) [, Pi (6)]
         if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
             const double* rq = S.ring + rslot(it + NS - 1) * BmeTraits::SLOT;
-            const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t), q2 = lds2(rq + 2 * PP + 2 * t),
-                          q3 = lds2(rq + 3 * PP + 2 * t), q4 = lds2(rq + 4 * PP + 2 * t);
-            o[0] = q0.x; o[3] = q0.y; o[1] = q1.x; o[2] = q1.y; o[4] = q2.x; o[5] = q2.y; o[6] = q3.x; o[7] = q3.y;
-            o[8] = q4.x; o[9] = q4.y;
+            const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
+            o[0] = q0.x; o[3] = q0.y; o[1] = q1.x; o[2] = q1.y;
+#pragma unroll
+            for (int P = 2; P < BmeTraits::NPAIR; ++P) {
+                const double2 qp = lds2(rq + P * PP + 2 * t);
+                o[2 * P] = qp.x; o[2 * P + 1] = qp.y;
+            }
         } else {
             o[0] = c.n;
 #pragma unroll
             for (int d = 0; d < 3; ++d) o[1 + d] = fma(-th2, Pz[d], c.acc[d]) * c.in;
 #pragma unroll
             for (int q = 0; q < 6; ++q) o[4 + q] = fma(-th4, EFz[q], c.acc[3 + q]);
+            if (OD) {
+                pi_source<2>(c.accP, c.Pi, usz, -th2);        // the upper z face completes Pi*(j)
+#pragma unroll
+                for (int q = 0; q < 6; ++q) o[PI0 + q] = c.accP[q];
+            }
         }
-        sts2(rs + 2 * t, o[0], o[3]); sts2(rs + PP + 2 * t, o[1], o[2]); sts2(rs + 2 * PP + 2 * t, o[4], o[5]);
-        sts2(rs + 3 * PP + 2 * t, o[6], o[7]); sts2(rs + 4 * PP + 2 * t, o[8], o[9]);
+        sts2(rs + 2 * t, o[0], o[3]); sts2(rs + PP + 2 * t, o[1], o[2]);
+#pragma unroll
+        for (int P = 2; P < BmeTraits::NPAIR; ++P) sts2(rs + P * PP + 2 * t, o[2 * P], o[2 * P + 1]);
         if (bot_dup) {                        // outflow: U*(-1) := U*(0)
             double* rg = S.ring + rslot(it + NS - 1) * BmeTraits::SLOT;
-            sts2(rg + 2 * t, o[0], o[3]); sts2(rg + PP + 2 * t, o[1], o[2]); sts2(rg + 2 * PP + 2 * t, o[4], o[5]);
-            sts2(rg + 3 * PP + 2 * t, o[6], o[7]); sts2(rg + 4 * PP + 2 * t, o[8], o[9]);
+            sts2(rg + 2 * t, o[0], o[3]); sts2(rg + PP + 2 * t, o[1], o[2]);
+#pragma unroll
+            for (int P = 2; P < BmeTraits::NPAIR; ++P) sts2(rg + P * PP + 2 * t, o[2 * P], o[2 * P + 1]);
         }
         if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
             const double2 wm = lds2(S.ring + rslot(it + NS - 2) * BmeTraits::SLOT + PP + 2 * t);
@@ -1039,13 +1180,18 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
     for (int d = 0; d < 3; ++d) c.u[d] = u_n[d];
 #pragma unroll
     for (int q = 0; q < 6; ++q) c.Pi[q] = Pi_n[q];
+    if (OD) {        // Pi*(j+1) starts from the carried tensor and the lower z face
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c.accP[q] = Pi_n[q];
+        pi_source<2>(c.accP, Pi_n, usz, th2);
+    }
     row_arrive_at<OP_OWN>(f.rowbar);                                  // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
         if (f.fix) {
 #pragma unroll
-            for (int P = 0; P < 5; ++P) {
+            for (int P = 0; P < BmeTraits::NPAIR; ++P) {
                 const double2 v = lds2(rs + P * PP + 2 * f.fix_src);
                 sts2(rs + P * PP + 2 * t, v.x, v.y);
                 if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + P * PP + 2 * t, v.x, v.y);
@@ -1060,13 +1206,13 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NBME>& a, BlockTab* T, 
 }
 
 __global__ void __launch_bounds__(NT, 1)
-k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
+k_fused_bme(const __grid_constant__ FusedArgs<NFB> a) {
     extern __shared__ __align__(128) unsigned char smraw[];
     BlockTab* T = reinterpret_cast<BlockTab*>(smraw);
     double* sm = reinterpret_cast<double*>(smraw + sizeof(BlockTab));
     BmeShared S;
     S.nu = sm; S.uu = sm + 2 * PL; S.px = sm + 4 * PL; S.py = sm + 6 * PL; S.pxy = sm + 8 * PL; S.phi = sm + 9 * PL;
-    S.fy = S.phi + NPHI * PL; S.ring = S.fy + 9 * PL; S.tz = S.ring + NS * BmeTraits::SLOT;
+    S.fy = S.phi + NPHI * PL; S.ring = S.fy + BmeTraits::NFY * PL; S.tz = S.ring + NS * BmeTraits::SLOT;
 
     const Geo& g = a.g;
     const Blk b = make_blk(g, a.zchunk);
@@ -1084,7 +1230,7 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
     const double tau = a.dt_ptr ? *a.dt_ptr : a.dt_val;
     const double th = tau / a.h, inv2h = 0.5 / a.h;
 
-    double smax = 0.0;
+    double smax = 0.0, kap = 0.0;
     int bad = 0;
     if (threadIdx.x >= NTE) {
 #if GP_REG_D
@@ -1092,7 +1238,7 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
 #endif
         LagRows L;
         lag_warps<BmeTraits>(a, T, b, S.ring, S.tz, S.phi, th, L);
-        smax = L.smax; bad = L.bad;
+        smax = L.smax; bad = L.bad; kap = L.kap;
     } else {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
@@ -1103,25 +1249,36 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
         {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
             int zm = map_safe(b.z0 - 2, g.nz, g.bcz);
             size_t off = f.base + (size_t)zm * f.nxny;
-            double U0[NBME];
+            double U0[NFB];
 #pragma unroll
-            for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][BSTR * off];
+            for (int q = 0; q < NFB; ++q) U0[q] = a.U[q][BSTR * off];
             const double n_a = U0[0];
             double in = frcp(n_a);
             const double u_a[3] = {U0[1] * in, U0[2] * in, U0[3] * in};
-            const double Pz_a[3] = {fma(-U0[1], u_a[2], U0[6]), fma(-U0[2], u_a[2], U0[8]), fma(-U0[3], u_a[2], U0[9])};
+            double Pz_a[3] = {fma(-U0[1], u_a[2], U0[6]), fma(-U0[2], u_a[2], U0[8]), fma(-U0[3], u_a[2], U0[9])};
+            if (OD) { Pz_a[0] = U0[PI0 + 2]; Pz_a[1] = U0[PI0 + 4]; Pz_a[2] = U0[PI0 + 5]; }   // carried Pi_xz, Pi_yz, Pi_zz
             zm = map_safe(b.z0 - 1, g.nz, g.bcz);
             off = f.base + (size_t)zm * f.nxny;
 #pragma unroll
-            for (int q = 0; q < NBME; ++q) U0[q] = a.U[q][BSTR * off];
+            for (int q = 0; q < NFB; ++q) U0[q] = a.U[q][BSTR * off];
             c.n = U0[0]; c.in = frcp(c.n);
 #pragma unroll
             for (int d = 0; d < 3; ++d) c.u[d] = U0[1 + d] * c.in;
-            c.Pi[0] = fma(-U0[1], c.u[0], U0[4]); c.Pi[1] = fma(-U0[1], c.u[1], U0[5]); c.Pi[2] = fma(-U0[1], c.u[2], U0[6]);
-            c.Pi[3] = fma(-U0[2], c.u[1], U0[7]); c.Pi[4] = fma(-U0[2], c.u[2], U0[8]); c.Pi[5] = fma(-U0[3], c.u[2], U0[9]);
+            if (OD) {
+#pragma unroll
+                for (int q = 0; q < 6; ++q) c.Pi[q] = U0[PI0 + q];
+            } else {
+                c.Pi[0] = fma(-U0[1], c.u[0], U0[4]); c.Pi[1] = fma(-U0[1], c.u[1], U0[5]); c.Pi[2] = fma(-U0[1], c.u[2], U0[6]);
+                c.Pi[3] = fma(-U0[2], c.u[1], U0[7]); c.Pi[4] = fma(-U0[2], c.u[2], U0[8]); c.Pi[5] = fma(-U0[3], c.u[2], U0[9]);
+            }
             const double Pr[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
-            double Pz[3], EFz[6];
-            bme_face<2>(n_a, u_a, Pz_a, c.n, c.u, Pr, Pz, EFz);
+            double Pz[3], EFz[6], usz[3];
+            bme_face<2>(n_a, u_a, Pz_a, c.n, c.u, Pr, Pz, EFz, usz);
+            if (OD) {
+#pragma unroll
+                for (int q = 0; q < 6; ++q) c.accP[q] = c.Pi[q];
+                pi_source<2>(c.accP, c.Pi, usz, 0.5 * th);
+            }
 #pragma unroll
             for (int d = 0; d < 3; ++d) c.acc[d] = fma(0.5 * th, Pz[d], U0[1 + d]);
 #pragma unroll
@@ -1137,7 +1294,7 @@ k_fused_bme(const __grid_constant__ FusedArgs<NBME> a) {
         for (; j <= b.z1 - 1; ++j) bme_iter<true>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1; ++j) bme_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
     }
-    block_max_commit(smax, bad, a.smax_bits, a.flag, S.nu);
+    block_max_commit(smax, bad, a.smax_bits, a.flag, S.nu, kap, a.kappa);
 }
 
 #endif  // GP_FUSED_BME
@@ -1188,12 +1345,13 @@ static bool encode_map(CUtensorMap* tm, const void* base, size_t row_doubles, si
 }
 
 template <int NF, class K>
-static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, double dt, const double* d_dt,
-                          const double* src_in = nullptr, double* src_out = nullptr) {
+static int launch_fused_t(gp_ctx* c, K kernel, const int* fields, int planes, int kid, double dt, const double* d_dt,
+                          const double* src_in = nullptr, double* src_out = nullptr, int balance = 0, double* kappa = nullptr) {
     FusedArgs<NF> a;
     a.src_in = src_in; a.src_out = src_out;
+    a.balance = balance; a.kappa = kappa;
     a.g = Geo{c->g.nx, c->g.ny, c->g.nz, c->bc.x, c->bc.y, c->bc.z};
-    for (int f = 0; f < NF; ++f) { a.U[f] = c->U[f0 + f]; a.Un[f] = c->Us[f0 + f]; }
+    for (int f = 0; f < NF; ++f) { a.U[f] = c->U[fields[f]]; a.Un[f] = c->Us[fields[f]]; }
     a.phi = phipad_of(c);
     bool ok = true;
     for (int P = 0; P < NF / 2; ++P) ok = ok && encode_map(&a.tm[P], a.U[2 * P], 2 * (size_t)c->g.nx, c->g.ny, c->g.nz, 2 * FX);
@@ -1217,17 +1375,23 @@ static int launch_fused_t(gp_ctx* c, K kernel, int f0, int planes, int kid, doub
 }
 
 #ifdef GP_FUSED_GAS
-static int launch_gas_impl(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out) {
-    return launch_fused_t<NGAS>(c, k_fused_gas, 0, GasTraits::PLANES, K_FUSED_GAS, dt, d_dt, src_in, src_out);
+static int launch_gas_impl(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out, int balance) {
+    const int fields[NGAS + NODG] = {0, 1, 2, 3, 4, F_EPS};
+    return launch_fused_t<NFG>(c, k_fused_gas, fields, GasTraits::PLANES, K_FUSED_GAS, dt, d_dt, src_in, src_out, balance,
+                               OD ? c->d_kappa : nullptr);
 }
 #endif
 #ifdef GP_FUSED_BME
-static int launch_bme_impl(gp_ctx* c, double dt, const double* d_dt) {
-    return launch_fused_t<NBME>(c, k_fused_bme, NGAS, BmeTraits::PLANES, K_FUSED_BME, dt, d_dt);
+static int launch_bme_impl(gp_ctx* c, double dt, const double* d_dt, int balance) {
+    int fields[NBME + NODB];
+    for (int f = 0; f < NBME; ++f) fields[f] = NGAS + f;
+    for (int q = 0; q < NODB; ++q) fields[NBME + q] = F_PI + q;
+    return launch_fused_t<NFB>(c, k_fused_bme, fields, BmeTraits::PLANES, K_FUSED_BME, dt, d_dt, nullptr, nullptr, balance,
+                               OD ? c->d_kappa + 1 : nullptr);
 }
 #endif
 
-#ifdef GP_FUSED_GAS
+#if defined(GP_FUSED_GAS) && !GP_OVERDET
 // evaluate the device reciprocal / reciprocal square root on n host-supplied values (self test)
 __global__ void k_math_selftest(int n, const double* __restrict__ x, double* __restrict__ rcp, double* __restrict__ rsq) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1251,14 +1415,22 @@ static int math_selftest_impl(int n, const double* x, double* rcp, double* rsq) 
 
 }  // namespace GP_FUSED_NS
 
-#ifdef GP_FUSED_GAS
+#if defined(GP_FUSED_GAS) && !GP_OVERDET
 int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out) {
-    return GP_FUSED_NS::launch_gas_impl(c, dt, d_dt, src_in, src_out);
+    return GP_FUSED_NS::launch_gas_impl(c, dt, d_dt, src_in, src_out, 0);
 }
 int math_selftest(int n, const double* x, double* rcp, double* rsq) { return GP_FUSED_NS::math_selftest_impl(n, x, rcp, rsq); }
 #endif
-#ifdef GP_FUSED_BME
-int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt) { return GP_FUSED_NS::launch_bme_impl(c, dt, d_dt); }
+#if defined(GP_FUSED_BME) && !GP_OVERDET
+int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt) { return GP_FUSED_NS::launch_bme_impl(c, dt, d_dt, 0); }
+#endif
+#if defined(GP_FUSED_GAS) && GP_OVERDET
+int launch_fused_gas_od(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out, int balance) {
+    return GP_FUSED_NS::launch_gas_impl(c, dt, d_dt, src_in, src_out, balance);
+}
+#endif
+#if defined(GP_FUSED_BME) && GP_OVERDET
+int launch_fused_bme_od(gp_ctx* c, double dt, const double* d_dt, int balance) { return GP_FUSED_NS::launch_bme_impl(c, dt, d_dt, balance); }
 #endif
 
 }  // namespace gp

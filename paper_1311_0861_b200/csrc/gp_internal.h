@@ -15,15 +15,28 @@ namespace gp {
 constexpr int NGAS = 5;
 constexpr int NBME = 10;
 constexpr int NHYD = NGAS + NBME;
+// Carried fields of the overdetermined system (GP_OD; PAPER.md:41 4th equation): rho*eps, Pi_ij (6).
+// Internal field index = public id - 1 (the public enum has GP_PHI between the two groups).
+constexpr int NODG = 1, NODB = 6;
+constexpr int F_EPS = NHYD, F_PI = NHYD + 1;
+constexpr int NALL = NHYD + NODG + NODB;
+inline int field_index(int public_id) { return public_id < NHYD ? public_id : public_id - 1; }
 // The state lives in HBM as arrays of field PAIRS, one double2 per cell: gas (rho,m_x) (m_y,m_z),
 // collisionless (n,nu_x) (nu_y,nu_z) (nE_xx,nE_xy) (nE_xz,nE_yy) (nE_yz,nE_zz), so that the fused
 // kernels stage and store 16 bytes per access straight into their paired shared-memory layout.
 // U[f] of a paired field points at its member of the pair and consecutive cells are BSTR doubles
-// apart.  The gas energy and Phi are plain arrays (stride 1).
+// apart.  The gas energy and Phi are plain arrays (stride 1) -- except in a GP_OD context, where the energy
+// is paired with the carried internal energy, (rho*E, rho*eps), and the carried Pi_ij form three more pairs
+// (Pi_xx,Pi_xy) (Pi_xz,Pi_yy) (Pi_yz,Pi_zz).  Indices below are internal (field_index).
 constexpr int BSTR = 2;
-constexpr int NGASP = 4;          // gas fields 0..3 are paired, field 4 (energy) is plain
-inline bool field_paired(int f) { return f < NGASP || (f >= NGAS && f < NHYD); }
-inline int pair_base(int f) { return f < NGAS ? (f & ~1) : NGAS + ((f - NGAS) & ~1); }
+constexpr int NGASP = 4;          // gas fields 0..3 are always paired
+inline bool field_paired(int f, bool od) { return f < NGASP || (f >= NGAS && f < NHYD) || (od && (f == NGAS - 1 || f >= NHYD)); }
+// the first member of the pair field f belongs to
+inline int pair_base(int f) {
+    if (f == NGAS - 1 || f == F_EPS) return NGAS - 1;
+    if (f > F_EPS) return F_PI + ((f - F_PI) & ~1);
+    return f < NGAS ? (f & ~1) : NGAS + ((f - NGAS) & ~1);
+}
 
 // Grid geometry handed to kernels by value.
 struct Geo {
@@ -58,7 +71,7 @@ void set_error(const char* fmt, ...);
 
 // Kernels (and cuFFT executions) that can be timed one by one with CUDA events.
 enum KernelId { K_CFL = 0, K_SOURCE, K_FFT_FWD, K_GREEN, K_FFT_INV, K_PHI_GHOST, K_PAD_SOURCE, K_MUL_KERNEL, K_EXTRACT,
-                K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_ISO_YFWD, K_ISO_ZFUSED, K_ISO_YINV, K_NUM };
+                K_FUSED_GAS, K_FUSED_BME, K_ZPASS, K_ISO_YFWD, K_ISO_ZFUSED, K_ISO_YINV, K_OD_AUX, K_NUM };
 
 struct Timing {
     bool on = false;
@@ -83,14 +96,18 @@ struct gp_ctx {
     size_t bytes;
     bool owns;
     bool ready;
-    double* U[gp::NHYD];    // state U^n
-    double* Us[gp::NHYD];   // target of the fused step (U^{n+1}); swapped with U after every step
+    bool od;                // GP_OD: the overdetermined system is carried (fields NHYD.. exist, the energy is paired)
+    int estr;               // stride of the gas energy array in doubles (1, or BSTR with GP_OD)
+    double* U[gp::NALL];    // state U^n (internal field index)
+    double* Us[gp::NALL];   // target of the fused step (U^{n+1}); swapped with U after every step
     double* phip;                   // Phi, padded by two ghost layers (PhiPad above)
     double* d_dt;                   // [0] = dt of the last gp_max_dt
     unsigned long long* d_smax;     // bit pattern of the running max signal speed
     int* d_flag;                    // != 0: bad state seen by the CFL reduction
     unsigned long long* d_smax_next;   // max signal speed of U^{n+1}, folded by the fused step kernels
     int* d_flag_next;
+    double* d_kappa;                // GP_OD: [0..1] kappa_gas, kappa_bme folded by the last step (before its balance), [2..3] of gp_kappa
+    bool kappa_cached;
     bool cfl_cached;                // d_smax_next / d_flag_next describe the current state
 
     // Poisson
@@ -136,6 +153,14 @@ int launch_strided_copy(gp_ctx* c, double* dst, int dstride, const double* src, 
 // src_out != nullptr: also write rho + n of the new state there (src_in = the new n, or nullptr)
 int launch_fused_gas(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out);
 int launch_fused_bme(gp_ctx* c, double dt, const double* d_dt);
+// fused_gas_od.cu, fused_bme_od.cu: the same kernels carrying the overdetermined system (GP_OD)
+int launch_fused_gas_od(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out, int balance);
+int launch_fused_bme_od(gp_ctx* c, double dt, const double* d_dt, int balance);
+
+// od.cu: cell-local passes of the overdetermined system
+int launch_od_derive(gp_ctx* c);
+int launch_od_balance(gp_ctx* c);
+int launch_od_kappa(gp_ctx* c, double* d_out);
 int math_selftest(int n, const double* x, double* rcp, double* rsq);
 
 // selftest.cu

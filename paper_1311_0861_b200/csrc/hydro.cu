@@ -16,14 +16,15 @@ __device__ __forceinline__ constexpr int sym(int i, int j) {
 
 struct GasPrim { double rho, v[3], p; };
 
-__device__ __forceinline__ GasPrim gas_prim(const ConstFields<NGAS>& U, size_t c, double gm1) {
+// estr: stride of the energy array (1, or BSTR in a GP_OD context where it is paired with rho*eps)
+__device__ __forceinline__ GasPrim gas_prim(const ConstFields<NGAS>& U, size_t c, double gm1, int estr) {
     GasPrim w;
     w.rho = U.p[0][BSTR * c];
     const double ir = 1.0 / w.rho;
     w.v[0] = U.p[1][BSTR * c] * ir;
     w.v[1] = U.p[2][BSTR * c] * ir;
     w.v[2] = U.p[3][BSTR * c] * ir;
-    w.p = gm1 * (U.p[4][c] - 0.5 * w.rho * (w.v[0] * w.v[0] + w.v[1] * w.v[1] + w.v[2] * w.v[2]));
+    w.p = gm1 * (U.p[4][estr * c] - 0.5 * w.rho * (w.v[0] * w.v[0] + w.v[1] * w.v[1] + w.v[2] * w.v[2]));
     return w;
 }
 
@@ -33,14 +34,14 @@ __device__ __forceinline__ GasPrim gas_prim(const ConstFields<NGAS>& U, size_t c
 // values and one atomicMax on the 64-bit pattern finishes the reduction.
 // --------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_cfl(size_t N, int has_gas, int has_stars, ConstFields<NGAS> Ug, ConstFields<NBME> Ub, double gamma,
+k_cfl(size_t N, int has_gas, int has_stars, ConstFields<NGAS> Ug, int estr, ConstFields<NBME> Ub, double gamma,
       unsigned long long* __restrict__ smax_bits, int* __restrict__ flag) {
     double smax = 0.0;
     int bad = 0;
     const double gm1 = gamma - 1.0;
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (size_t)gridDim.x * blockDim.x) {
         if (has_gas) {
-            const GasPrim w = gas_prim(Ug, c, gm1);
+            const GasPrim w = gas_prim(Ug, c, gm1, estr);
             if (!(w.rho > 0.0) || !(w.p > 0.0)) bad = 1;
             const double cs = sqrt(gamma * w.p / w.rho);
 #pragma unroll
@@ -163,7 +164,7 @@ int launch_cfl(gp_ctx* c, double cfl) {
     size_t blocks = (c->N + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
     k_cfl<<<(unsigned)blocks, 256, 0, c->stream>>>(c->N, (c->g.components & GP_GAS) != 0, (c->g.components & GP_STARS) != 0,
-                                                   Ug, Ub, c->gamma, c->d_smax, c->d_flag);
+                                                   Ug, c->estr, Ub, c->gamma, c->d_smax, c->d_flag);
     k_cfl_finish<<<1, 1, 0, c->stream>>>(c->d_smax, c->d_flag, c->d_flag, cfl, c->g.h, c->d_dt);
     toc(c);
     c->n_own += 3;
