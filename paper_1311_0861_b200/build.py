@@ -20,7 +20,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps)):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--threads", "0",
            "-shared", "-Xcompiler", "-fPIC", "-o", LIB] + os.environ.get("GP_NVCC_FLAGS", "").split() + sources() + ["-lcufft"]
     if verbose:
         cmd.insert(1, "-Xptxas")
