@@ -12,6 +12,12 @@
 // through shared memory.  ZC adjacent columns (ZC * 16 B contiguous in HBM) share a block.
 #include "fftcol.cuh"
 
+// columns per block and blocks per SM of the 512-point pass (the headline size)
+#ifndef GP_ZP9_C
+#define GP_ZP9_C 4
+#define GP_ZP9_MINB 2
+#endif
+
 namespace gp {
 
 // forward stages s..S-1, Green multiply, inverse stages S-1..s (compile-time recursion)
@@ -100,7 +106,7 @@ int launch_zpass(gp_ctx* c, double coef6) {
         case 64: return launch_zpass_t<6, 8, 1>(c, coef6);
         case 128: return launch_zpass_t<7, 8, 1>(c, coef6);
         case 256: return launch_zpass_t<8, 8, 1>(c, coef6);
-        case 512: return launch_zpass_t<9, 4, 2>(c, coef6);   // two 256-thread blocks per SM beat one of 512
+        case 512: return launch_zpass_t<9, GP_ZP9_C, GP_ZP9_MINB>(c, coef6);   // two 256-thread blocks per SM beat one of 512
         case 1024: return launch_zpass_t<10, 4, 1>(c, coef6);
     }
     set_error("launch_zpass: nz = %d is not a supported power of two", c->g.nz);
