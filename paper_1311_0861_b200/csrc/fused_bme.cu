@@ -14,6 +14,14 @@
 #define GP_NDW GP_BME_NDW
 #define GP_REG_E GP_BME_REG_E
 #define GP_REG_D GP_BME_REG_D
+#ifndef GP_BME_TZREG
+#define GP_BME_TZREG 0
+#endif
+#define GP_TZREG GP_BME_TZREG
+#ifndef GP_BME_YRECOMP
+#define GP_BME_YRECOMP 0
+#endif
+#define GP_YRECOMP GP_BME_YRECOMP
 #define GP_FUSED_NS fbme
 #define GP_FUSED_BME 1
 #include "fused_impl.cuh"

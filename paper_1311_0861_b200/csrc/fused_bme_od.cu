@@ -16,6 +16,14 @@
 #define GP_NDW GP_BMEOD_NDW
 #define GP_REG_E GP_BMEOD_REG_E
 #define GP_REG_D GP_BMEOD_REG_D
+#ifndef GP_BMEOD_TZREG
+#define GP_BMEOD_TZREG 0
+#endif
+#define GP_TZREG GP_BMEOD_TZREG
+#ifndef GP_BMEOD_YRECOMP
+#define GP_BMEOD_YRECOMP 0
+#endif
+#define GP_YRECOMP GP_BMEOD_YRECOMP
 #define GP_FUSED_NS fbmeod
 #define GP_FUSED_BME 1
 #include "fused_impl.cuh"

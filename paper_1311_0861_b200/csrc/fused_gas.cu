@@ -17,6 +17,10 @@
 #define GP_NDW GP_GAS_NDW
 #define GP_REG_E GP_GAS_REG_E
 #define GP_REG_D GP_GAS_REG_D
+#ifndef GP_GAS_TZREG
+#define GP_GAS_TZREG 0
+#endif
+#define GP_TZREG GP_GAS_TZREG
 #define GP_FUSED_NS fgas
 #define GP_FUSED_GAS 1
 #include "fused_impl.cuh"

@@ -18,6 +18,10 @@
 #define GP_NDW GP_GASOD_NDW
 #define GP_REG_E GP_GASOD_REG_E
 #define GP_REG_D GP_GASOD_REG_D
+#ifndef GP_GASOD_TZREG
+#define GP_GASOD_TZREG 0
+#endif
+#define GP_TZREG GP_GASOD_TZREG
 #define GP_FUSED_NS fgasod
 #define GP_FUSED_GAS 1
 #include "fused_impl.cuh"

@@ -66,6 +66,20 @@ constexpr int DROWS = TYO / NDW;          // output rows per Lagrangian warp
 #define GP_OVERDET 0
 #endif
 constexpr bool OD = GP_OVERDET != 0;
+// GP_TZREG: the Eulerian threads keep w*_x, w*_y of their own column of the last two planes in registers for the
+// z-averaged face-velocity plane instead of reading them back from the ring (32 bytes of shared-memory traffic less
+// per thread and plane, 8 registers more)
+#ifndef GP_TZREG
+#define GP_TZREG 0
+#endif
+constexpr bool TZREG = GP_TZREG != 0;
+// GP_YRECOMP (collisionless kernel): every Eulerian row solves BOTH its y faces (the lower one from the primitives of
+// the row below) instead of taking the lower face's fluxes from the row below through shared memory: one face solve
+// more per cell, 88 bytes of exchange and one row hand-off per plane less, three independent solver chains in stage B
+#ifndef GP_YRECOMP
+#define GP_YRECOMP 0
+#endif
+constexpr bool YRECOMP = GP_YRECOMP != 0;
 constexpr int NS = GP_NS;                 // slots of the U* ring: planes j-2, j-1, j of the Lagrangian warps and NS - 3 ahead
 constexpr int NPHI = NS + 2;              // slots of the Phi ring
 constexpr int NTZ = NS - 2;               // buffers of the z-averaged face-velocity plane
@@ -489,7 +503,7 @@ struct Foot {
     unsigned rowbar;     // shared address of yrdy[ty - 1]; the row's other hand-off barriers sit at the offsets below
 };
 // byte offsets from Foot::rowbar: y fluxes of the row below / of this row, primitives of this row / of the row above
-constexpr int OY_LO = 0, OY_OWN = 8, OP_OWN = 8 + 8 * FY, OP_UP = 16 + 8 * FY;
+constexpr int OY_LO = 0, OY_OWN = 8, OY_UP = 16, OP_LO = 8 * FY, OP_OWN = 8 + 8 * FY, OP_UP = 16 + 8 * FY;
 static_assert(offsetof(BlockTab, landed) == 0 && offsetof(BlockTab, ufull) == 8 * NS, "ring barriers are addressed from the table base");
 static_assert(offsetof(BlockTab, prdy) == offsetof(BlockTab, yrdy) + 8 * FY, "row barriers are addressed from yrdy");
 
@@ -702,6 +716,7 @@ struct GasCarry {
     double rho, ir, vx, vy, vz, p;        // primitives of the current plane j (own cell)
     double amx, amy, amz, aE;             // U*(j) under construction
     double eps, adv;                      // GP_OD: rho*eps of plane j; 2 x (sum of V_hi - V_lo over the faces done so far)
+    double wxm, wym, wx0, wy0;            // GP_TZREG: w*_x, w*_y of planes j-2 and j-1
 };
 
 struct GasShared {
@@ -807,9 +822,17 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, c
             if (OD) sts2(rg + 2 * PP + 2 * t, Es, epss); else rg[2 * PP + t] = Es;
         }
         if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
-            const double2 wm = lds2(S.ring + rslot(it + NS - 2) * GasTraits::SLOT + PP + 2 * t);
-            const double2 w0 = lds2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + PP + 2 * t);
-            sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, w0.x, wx), sum3(wm.y, w0.y, wy));
+            if (TZREG) {
+                sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(c.wxm, c.wx0, wx), sum3(c.wym, c.wy0, wy));
+            } else {
+                const double2 wm = lds2(S.ring + rslot(it + NS - 2) * GasTraits::SLOT + PP + 2 * t);
+                const double2 w0 = lds2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + PP + 2 * t);
+                sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, w0.x, wx), sum3(wm.y, w0.y, wy));
+            }
+        }
+        if (TZREG) {
+            c.wxm = bot_dup ? wx : c.wx0; c.wym = bot_dup ? wy : c.wy0;
+            c.wx0 = wx; c.wy0 = wy;
         }
     }
     sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
@@ -988,6 +1011,7 @@ struct BmeCarry {
     double n, in, u[3], Pi[6];            // primitives of the current plane j (own cell)
     double acc[9];                        // U*(j) under construction: nu (3), nE (6)
     double accP[6];                       // GP_OD: Pi*(j) under construction
+    double wxm, wym, wx0, wy0;            // GP_TZREG: w*_x, w*_y of planes j-2 and j-1
 };
 
 // y-flux exchange of one cell: Py (3), EFy (6) and, under GP_OD, 2u* (3)
@@ -1027,7 +1051,55 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
     const int it = j - (b.z0 - 1);
     const double* ph0 = S.phi + pslot(it + 1) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
     if (it > 0 && f.ty < FY - 1) mbar_wait_at<OP_UP>(f.rowbar, (it - 1) & 1);   // primitives of plane j of the row above are published
+    if (YRECOMP && it > 0 && f.ty > 0) mbar_wait_at<OP_LO>(f.rowbar, (it - 1) & 1);   // ... and of the row below
 
+  if (YRECOMP) {
+    // B + C in one basic block: x face (hi; lo from the left lane), BOTH y faces, flux differences, gravity source
+    if (f.star_row) {
+        const int tn = t + FX, ts = t - FX, te = f.tx < FX - 1 ? t + 1 : t;
+        const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
+        const double2 z0 = lds2(S.nu + 2 * ts), z1 = lds2(S.uu + 2 * ts), z2 = lds2(S.py + 2 * ts);
+        const double2 x0 = lds2(S.nu + 2 * te), x1 = lds2(S.uu + 2 * te), x2 = lds2(S.px + 2 * te);
+        const double pxy_n = S.pxy[tn], pxy_s = S.pxy[ts], pxy_e = S.pxy[te];
+        const double ury[3] = {y0.y, y1.x, y1.y}, uly[3] = {z0.y, z1.x, z1.y}, urx[3] = {x0.y, x1.x, x1.y};
+        const double Pcy[3] = {c.Pi[1], c.Pi[3], c.Pi[4]}, Plx[3] = {c.Pi[0], c.Pi[1], c.Pi[2]};
+        const double Pry[3] = {pxy_n, y2.x, y2.y}, Pby[3] = {pxy_s, z2.x, z2.y}, Prx[3] = {x2.x, pxy_e, x2.y};
+        double Py[3], EFy[6], usy[3], Pyl[3], EFyl[6], usyl[3], Px[3], EFx[6], usx[3];
+        bme_face<1>(c.n, c.u, Pcy, y0.x, ury, Pry, Py, EFy, usy);
+        bme_face<1>(z0.x, uly, Pby, c.n, c.u, Pcy, Pyl, EFyl, usyl);
+        bme_face<0>(c.n, c.u, Plx, x0.x, urx, Prx, Px, EFx, usx);
+        if (OD) {
+            double du2[3];
+#pragma unroll
+            for (int q = 0; q < 3; ++q) du2[q] = usx[q] - __shfl_up_sync(0xffffffffu, usx[q], 1);
+            pi_source<0>(c.accP, c.Pi, du2, -th2);
+#pragma unroll
+            for (int q = 0; q < 3; ++q) du2[q] = usy[q] - usyl[q];
+            pi_source<1>(c.accP, c.Pi, du2, -th2);
+        }
+#pragma unroll
+        for (int q = 0; q < 3; ++q) c.acc[q] -= th2 * ((Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1)) + (Py[q] - Pyl[q]));
+#pragma unroll
+        for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th4 * ((EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1)) + (EFy[q] - EFyl[q]));
+        // gravity (reading G5): -tau n g_i and -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
+        const double gr[3] = {(ph0[te] - ph0[f.tx > 0 ? t - 1 : t]) * inv2h, (ph0[tn] - ph0[ts]) * inv2h,
+                              (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h};
+        double uc[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], c.u[d]);
+        const double tn_ = tau * c.n;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c.acc[d] = fma(-tn_, gr[d], c.acc[d]);
+        c.acc[3] = fma(-tn_, 2.0 * uc[0] * gr[0], c.acc[3]);
+        c.acc[4] = fma(-tn_, fma(uc[0], gr[1], uc[1] * gr[0]), c.acc[4]);
+        c.acc[5] = fma(-tn_, fma(uc[0], gr[2], uc[2] * gr[0]), c.acc[5]);
+        c.acc[6] = fma(-tn_, 2.0 * uc[1] * gr[1], c.acc[6]);
+        c.acc[7] = fma(-tn_, fma(uc[1], gr[2], uc[2] * gr[1]), c.acc[7]);
+        c.acc[8] = fma(-tn_, 2.0 * uc[2] * gr[2], c.acc[8]);
+    }
+    // the neighbours' primitives of plane j are in registers: rows above and below may publish those of plane j+1
+    row_arrive_at<OY_OWN>(f.rowbar);
+  } else {
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
     // dependent chains interleave
     double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, usy[3] = {0.0, 0.0, 0.0};
@@ -1101,6 +1173,8 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         c.acc[8] = fma(-tn, 2.0 * uc[2] * gr[2], c.acc[8]);
     }
 
+  }
+
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
     // publish primitives(j+1)
     double* rs = S.ring + rslot(it) * BmeTraits::SLOT;
@@ -1164,10 +1238,22 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
             for (int P = 2; P < BmeTraits::NPAIR; ++P) sts2(rg + P * PP + 2 * t, o[2 * P], o[2 * P + 1]);
         }
         if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
-            const double2 wm = lds2(S.ring + rslot(it + NS - 2) * BmeTraits::SLOT + PP + 2 * t);
-            const double2 w0 = lds2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + PP + 2 * t);
-            sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, w0.x, o[1]), sum3(wm.y, w0.y, o[2]));
+            if (TZREG) {
+                sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(c.wxm, c.wx0, o[1]), sum3(c.wym, c.wy0, o[2]));
+            } else {
+                const double2 wm = lds2(S.ring + rslot(it + NS - 2) * BmeTraits::SLOT + PP + 2 * t);
+                const double2 w0 = lds2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + PP + 2 * t);
+                sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, w0.x, o[1]), sum3(wm.y, w0.y, o[2]));
+            }
         }
+        if (TZREG) {
+            c.wxm = bot_dup ? o[1] : c.wx0; c.wym = bot_dup ? o[2] : c.wy0;
+            c.wx0 = o[1]; c.wy0 = o[2];
+        }
+    }
+    if (YRECOMP) {       // the rows below and above have read the primitives of plane j
+        if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);
+        if (f.ty < FY - 1) mbar_wait_at<OY_UP>(f.rowbar, it & 1);
     }
     sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
     sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];

@@ -55,3 +55,29 @@ def test_product_path_does_not_touch_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
                 assert "liboracle" not in text and "oracle.h" not in text, f
+
+
+def test_binding_constants_match_the_header():
+    """Field ids, component bits and error codes of the ctypes binding are those of include/gpupegas.h."""
+    from paper_1311_0861_b200 import binding as B
+    text = open(os.path.join(ROOT, "include", "gpupegas.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    values = {}
+    for body in re.findall(r"enum\s*\{(.*?)\}", text, flags=re.S):
+        nxt = 0
+        for item in [x.strip() for x in body.split(",") if x.strip()]:
+            name, _, val = [p.strip() for p in item.partition("=")]
+            if val:
+                nxt = values[val] if val in values else int(val, 0)
+            values[name] = nxt
+            nxt += 1
+    names = ["RHO", "MX", "MY", "MZ", "E", "N", "NUX", "NUY", "NUZ", "EXX", "EXY", "EXZ", "EYY", "EYZ", "EZZ", "PHI",
+             "EPS", "PXX", "PXY", "PXZ", "PYY", "PYZ", "PZZ"]
+    order = B.FIELDS + B.OD_GAS_FIELDS + B.OD_STAR_FIELDS
+    assert len(order) == len(names) == values["GP_NFIELDS_OD"]
+    for py_name, c_name in zip(order, names):
+        assert B.FIELD_ID[py_name] == values["GP_" + c_name], (py_name, c_name)
+    assert (B.GP_GAS, B.GP_STARS, B.GP_OD) == (values["GP_GAS"], values["GP_STARS"], values["GP_OD"])
+    assert (B.GP_ERR_STATE, B.GP_ERR_UNSUPPORTED) == (values["GP_ERR_STATE"], values["GP_ERR_UNSUPPORTED"])
+    assert (B.GP_POISSON_PERIODIC, B.GP_POISSON_ISOLATED, B.GP_BC_OUTFLOW) == (
+        values["GP_POISSON_PERIODIC"], values["GP_POISSON_ISOLATED"], values["GP_BC_OUTFLOW"])
