@@ -17,8 +17,9 @@
 #define GP_NDW GP_GAS_NDW
 #define GP_REG_E GP_GAS_REG_E
 #define GP_REG_D GP_GAS_REG_D
+// w*_x, w*_y of the last two planes stay in registers for the z-averaged face-velocity plane: 5.87 -> 5.54 ms
 #ifndef GP_GAS_TZREG
-#define GP_GAS_TZREG 0
+#define GP_GAS_TZREG 1
 #endif
 #define GP_TZREG GP_GAS_TZREG
 #define GP_FUSED_NS fgas
