@@ -141,7 +141,7 @@ static int ensure_storage(gp_ctx* c) {
             c->U[NGAS + 2 * P] = u; c->U[NGAS + 2 * P + 1] = u + 1;
             c->Us[NGAS + 2 * P] = us; c->Us[NGAS + 2 * P + 1] = us + 1;
         }
-    c->phip = (double*)take(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double));
+    c->phip = (double*)take(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double)) + (PHI_XOFF - 2);   // interior rows 128-byte aligned
     c->d_kappa = (double*)take(256);
     c->kappa_cached = false;
     char* small = take(256);

@@ -55,7 +55,7 @@ struct ConstFields {
 };
 
 // Phi lives in an array padded by TWO ghost layers per side: cell (i,j,k), i in [-2, nx+1] etc., sits at
-// p[(i+2) + pitch*((j+2) + py*(k+2))], pitch = nx+4 rounded up to even (rows stay 16-byte aligned), py = ny+4.
+// p[(i+2) + pitch*((j+2) + py*(k+2))], pitch >= nx+4 (phi_pitch below), py = ny+4.
 // Layer 1 holds the ghost values of the Poisson mode (periodic solve: wrapped; isolated solve: the padded
 // convolution at indices -1 and n; user-set Phi: the hydro rule per axis); layer 2, edges and corners are
 // index maps of the same rule (wrap, or clamp for the isolated solve) and are only ever read for the U* of
@@ -64,8 +64,12 @@ struct PhiPad {
     const double* p;
     int pitch, py;
 };
-inline int phi_pitch(int nx) { return (nx + 4 + 1) & ~1; }
-inline size_t phi_pad_elems(int nx, int ny, int nz) { return (size_t)phi_pitch(nx) * (ny + 4) * (nz + 4); }
+// The array is laid out so that the interior rows (the rows the inverse transform writes and the kernels read most)
+// start on 128-byte boundaries: the first ghost column sits PHI_XOFF - 2 doubles into a 256-byte aligned allocation,
+// the pitch is a multiple of 16 doubles.  gp_ctx::phip points at the first ghost column.
+constexpr int PHI_XOFF = 16;
+inline int phi_pitch(int nx) { return (nx + PHI_XOFF + 2 + 15) & ~15; }
+inline size_t phi_pad_elems(int nx, int ny, int nz) { return (size_t)phi_pitch(nx) * (ny + 4) * (nz + 4) + PHI_XOFF; }
 
 void set_error(const char* fmt, ...);
 
