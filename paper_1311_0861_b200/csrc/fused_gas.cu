@@ -22,6 +22,11 @@
 #define GP_GAS_TZREG 1
 #endif
 #define GP_TZREG GP_GAS_TZREG
+// stage E publishes the primitives of the next plane before its z face solve: 5.53 -> 5.43 ms
+#ifndef GP_GAS_EARLYPUB
+#define GP_GAS_EARLYPUB 1
+#endif
+#define GP_EARLYPUB GP_GAS_EARLYPUB
 #define GP_FUSED_NS fgas
 #define GP_FUSED_GAS 1
 #include "fused_impl.cuh"

@@ -80,6 +80,12 @@ constexpr bool TZREG = GP_TZREG != 0;
 #define GP_YRECOMP 0
 #endif
 constexpr bool YRECOMP = GP_YRECOMP != 0;
+// GP_EARLYPUB: stage E publishes the primitives of plane j+1 (and releases the rows waiting for them) as soon as they
+// are recovered, before the z face solve and the U* stores, instead of at the end of the stage
+#ifndef GP_EARLYPUB
+#define GP_EARLYPUB 0
+#endif
+constexpr bool EARLYPUB = GP_EARLYPUB != 0;
 constexpr int NS = GP_NS;                 // slots of the U* ring: planes j-2, j-1, j of the Lagrangian warps and NS - 3 ahead
 constexpr int NPHI = NS + 2;              // slots of the Phi ring
 constexpr int NTZ = NS - 2;               // buffers of the z-averaged face-velocity plane
@@ -203,8 +209,17 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, uns
 // Wait for the phase of given parity of the mbarrier at shared address base + OFF (bytes; an immediate, so that no
 // second address register stays live across the loop).  try_wait suspends the warp for up to the hinted time, so a
 // waiting warp issues a poll only now and then instead of spinning on the issue port of the working warps.
+// GP_WAIT_MODE: 0 = try_wait in a plain loop, 1 = try_wait with a suspend-time hint (ptxas adds NANOSLEEP.SYNCS),
+// 2 = try_wait, then an explicit nanosleep of GP_WAIT_NS before the next try
+#ifndef GP_WAIT_MODE
+#define GP_WAIT_MODE 1
+#endif
+#ifndef GP_WAIT_NS
+#define GP_WAIT_NS 40
+#endif
 template <int OFF = 0>
 __device__ __forceinline__ void mbar_wait_at(unsigned base, unsigned parity) {
+#if GP_WAIT_MODE == 1
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "W_%=:\n\t"
@@ -213,6 +228,27 @@ __device__ __forceinline__ void mbar_wait_at(unsigned base, unsigned parity) {
         "bra W_%=;\n\t"
         "D_%=:\n\t}" ::"r"(base), "r"(parity), "r"(0x989680), "n"(OFF)
         : "memory");
+#elif GP_WAIT_MODE == 0
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "W_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%2], %1;\n\t"
+        "@p bra D_%=;\n\t"
+        "bra W_%=;\n\t"
+        "D_%=:\n\t}" ::"r"(base), "r"(parity), "n"(OFF)
+        : "memory");
+#else
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%2], %1;\n\t"
+        "@p bra D_%=;\n\t"
+        "W_%=:\n\t"
+        "nanosleep.u32 %3;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%2], %1;\n\t"
+        "@!p bra W_%=;\n\t"
+        "D_%=:\n\t}" ::"r"(base), "r"(parity), "n"(OFF), "n"(GP_WAIT_NS)
+        : "memory");
+#endif
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) { mbar_wait_at<0>(smem_u32(b), parity); }
 template <int OFF = 0>
@@ -794,6 +830,10 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, c
     const double vx_n = mx_n * ir_n, vy_n = my_n * ir_n, vz_n = mz_n * ir_n;
     // GP_OD: the pressure comes from the carried internal energy (4th equation)
     const double p_n = OD ? gm1 * eps_n : gm1 * (E_n - 0.5 * fma(mx_n, vx_n, fma(my_n, vy_n, mz_n * vz_n)));
+    if (EARLYPUB) {
+        sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
+        row_arrive_at<OP_OWN>(f.rowbar);                              // primitives of plane j+1 of this row are published
+    }
     double Pz = 0.0, PVz = 0.0, Vz = 0.0;
     if (f.star_row) {
         gas_face(gamma, c.rho, c.vz, c.p, rho_n, vz_n, p_n, Pz, PVz, Vz);
@@ -835,11 +875,11 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, c
             c.wx0 = wx; c.wy0 = wy;
         }
     }
-    sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n;
+    if (!EARLYPUB) { sts2(S.rp + 2 * t, rho_n, p_n); S.vx[t] = vx_n; S.vy[t] = vy_n; }
     c.amx = mx_n; c.amy = my_n; c.amz = fma(th2, Pz, mz_n); c.aE = fma(th4, PVz, E_n);
     c.rho = rho_n; c.ir = ir_n; c.vx = vx_n; c.vy = vy_n; c.vz = vz_n; c.p = p_n;
     if (OD) { c.eps = eps_n; c.adv = -Vz; }
-    row_arrive_at<OP_OWN>(f.rowbar);                                  // primitives of plane j+1 of this row are published
+    if (!EARLYPUB) row_arrive_at<OP_OWN>(f.rowbar);                   // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
@@ -1201,6 +1241,11 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         Pi_n[0] = fma(-Un[1], u_n[0], Un[4]); Pi_n[1] = fma(-Un[1], u_n[1], Un[5]); Pi_n[2] = fma(-Un[1], u_n[2], Un[6]);
         Pi_n[3] = fma(-Un[2], u_n[1], Un[7]); Pi_n[4] = fma(-Un[2], u_n[2], Un[8]); Pi_n[5] = fma(-Un[3], u_n[2], Un[9]);
     }
+    if (EARLYPUB && !YRECOMP) {
+        sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
+        sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];
+        row_arrive_at<OP_OWN>(f.rowbar);                              // primitives of plane j+1 of this row are published
+    }
     double Pz[3] = {0.0, 0.0, 0.0}, EFz[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, usz[3] = {0.0, 0.0, 0.0};
     if (f.star_row) {
         const double Pl[3] = {c.Pi[2], c.Pi[4], c.Pi[5]};
@@ -1255,8 +1300,10 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);
         if (f.ty < FY - 1) mbar_wait_at<OY_UP>(f.rowbar, it & 1);
     }
-    sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
-    sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];
+    if (!(EARLYPUB && !YRECOMP)) {
+        sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
+        sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];
+    }
 #pragma unroll
     for (int d = 0; d < 3; ++d) c.acc[d] = fma(th2, Pz[d], Un[1 + d]);
 #pragma unroll
@@ -1271,7 +1318,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         for (int q = 0; q < 6; ++q) c.accP[q] = Pi_n[q];
         pi_source<2>(c.accP, Pi_n, usz, th2);
     }
-    row_arrive_at<OP_OWN>(f.rowbar);                                  // primitives of plane j+1 of this row are published
+    if (!(EARLYPUB && !YRECOMP)) row_arrive_at<OP_OWN>(f.rowbar);     // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
