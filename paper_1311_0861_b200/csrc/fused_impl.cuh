@@ -15,25 +15,30 @@
 //          primitives, z face (j, j+1), complete U*(j) and write it (density, w* = momentum*/
 //          density, remaining fields) over the staged data -- U* never goes to HBM -- and publish
 //          the primitives of plane j+1 for the next B.
-//     Rows synchronise with their two neighbours only (named barriers of 64 threads, row_arrive / row_wait).
-//   * 4 Lagrangian warps ("D", one warpgroup; each serves (FY-4)/4 output rows).  Per plane j they
-//     wait for U*(j), advect plane j-1 from the four-slot U* ring (4-vertex face velocities as
+//     Rows synchronise with their two neighbours only, through two mbarriers per row (row_arrive_at /
+//     mbar_wait_at: "y fluxes written", "primitives published"); there is no block-wide barrier in the loop.
+//   * NDW Lagrangian warps ("D"; each serves (FY-4)/NDW output rows, one in the shipped builds).  Per plane j
+//     they wait for U*(j), advect plane j-1 from the NS-slot U* ring (4-vertex face velocities as
 //     separable (1/4,1/2,1/4) averages, upwind donor-cell fluxes in coefficient form), write
 //     U^{n+1}(j-1) to HBM and fold its max signal speed.  They also PRODUCE: as soon as all of them
-//     are done with the oldest ring slot, plane j+3 (and Phi(j+4)) is requested into it: one thread
+//     are done with the oldest ring slot, plane j+NS-1 (and Phi(j+NS)) is requested into it: one thread
 //     issues one TMA tensor copy (cp.async.bulk.tensor, a 32 x FY x 1 box) per field pair, completing
 //     on an mbarrier with a transaction count; no compute thread issues or waits for a copy
 //     instruction.  TMA cannot wrap or clamp, so blocks whose footprint reaches over the edge of
 //     the grid (and grids with odd nx, whose rows are not 16-byte aligned) stage cell by cell with
 //     cp.async on the same mbarrier.
-//   * E -> D hand-off: one mbarrier per ring slot ("U*(j) complete"), arrived on by one E thread
-//     after the E barrier.  D -> E: the "landed" mbarrier of the slot.  The E group runs up to two
-//     planes ahead of the D group.  Registers are split between the groups with setmaxnreg.
+//   * E -> D hand-off: one mbarrier per ring slot ("U*(j) complete"), arrived on by one lane of every
+//     E warp.  D -> E: the "landed" mbarrier of the slot.  The E group runs up to NS-3 planes ahead of
+//     the D group.  Registers are split between the groups with setmaxnreg.
 //
 // Ghost cells are index maps (wrap / clamp of the source row, plane or x segment); for outflow the U*
 // ghosts are copies of the nearest interior U* (H6), restored in shared memory after E.
 // Phi comes from an array padded by two ghost layers (gp_internal.h, PhiPad), filled by the rule of
 // the Poisson mode, so its staging needs no case analysis.
+//
+// Build parameters (set per translation unit by fused_gas.cu, fused_bme.cu and their _od twins): GP_FY, GP_NDW,
+// GP_NS, GP_REG_E / GP_REG_D, GP_OVERDET, GP_TZREG, GP_EARLYPUB, GP_YRECOMP, GP_WAIT_MODE; the measured effect of
+// each is recorded in DESIGN.md section 8.
 #include <cuda.h>
 
 #include <cstddef>
