@@ -81,3 +81,28 @@ def test_binding_constants_match_the_header():
     assert (B.GP_ERR_STATE, B.GP_ERR_UNSUPPORTED) == (values["GP_ERR_STATE"], values["GP_ERR_UNSUPPORTED"])
     assert (B.GP_POISSON_PERIODIC, B.GP_POISSON_ISOLATED, B.GP_BC_OUTFLOW) == (
         values["GP_POISSON_PERIODIC"], values["GP_POISSON_ISOLATED"], values["GP_BC_OUTFLOW"])
+
+
+def test_storage_accounting_is_host_arithmetic():
+    """gp_storage_bytes needs no device: state x 2 (ping-pong) + padded Phi + Poisson work arrays; a GP_OD context
+    adds two copies of its seven carried fields."""
+    import paper_1311_0861_b200 as pkg
+    B = pkg.binding
+    L = pkg.lib()
+
+    def nbytes(n, comp, poisson):
+        g = B.gp_grid(n, n, n, 1.0 / n, comp, poisson, 1.0)
+        return L.gp_storage_bytes(ctypes.byref(g))
+
+    n = 64
+    cell = 8 * n ** 3
+    gas, both = nbytes(n, B.GP_GAS, 0), nbytes(n, B.GP_GAS | B.GP_STARS, 0)
+    assert 2 * 5 * cell <= gas <= 2 * 5 * cell + 1.2 * 8 * (n + 34) * (n + 4) ** 2 + (1 << 16)
+    assert abs((both - gas) - 2 * 10 * cell) <= 1 << 16
+    od = nbytes(n, B.GP_GAS | B.GP_STARS | B.GP_OD, 0)
+    assert abs((od - both) - 2 * 7 * cell) <= 1 << 16
+    per = nbytes(n, B.GP_GAS | B.GP_STARS, B.GP_POISSON_PERIODIC)
+    assert per - both >= 16 * (n // 2 + 1) * n * n + cell          # half spectrum + the source rho + n
+    iso = nbytes(n, B.GP_GAS, B.GP_POISSON_ISOLATED)
+    assert iso > gas + 4 * cell
+    assert L.gp_storage_bytes(None) == 0
