@@ -6,7 +6,11 @@
 #define GP_GAS_NDW 12
 #endif
 #ifndef GP_GAS_REG_E
+#if defined(GP_GAS_EROWS) && GP_GAS_EROWS == 2
+#define GP_GAS_REG_E 152
+#else
 #define GP_GAS_REG_E 80
+#endif
 #define GP_GAS_REG_D 56
 #endif
 #ifndef GP_GAS_NS
@@ -27,6 +31,11 @@
 #define GP_GAS_EARLYPUB 1
 #endif
 #define GP_EARLYPUB GP_GAS_EARLYPUB
+// two footprint rows per Eulerian thread (8 + 12 warps, 640 threads launched at 96 registers, 152 / 56 after the split)
+#ifndef GP_GAS_EROWS
+#define GP_GAS_EROWS 1
+#endif
+#define GP_EROWS GP_GAS_EROWS
 #define GP_FUSED_NS fgas
 #define GP_FUSED_GAS 1
 #include "fused_impl.cuh"

@@ -56,7 +56,14 @@ constexpr int TXO = FX - 4, TYO = FY - 4;
 #ifndef GP_NDW
 #define GP_NDW 8
 #endif
-constexpr int NEW = FY;                   // Eulerian warps, one per footprint row
+// GP_EROWS: footprint rows per Eulerian warp (1, or 2 adjacent rows per thread in the gas kernel: the y face between
+// the two rows stays in registers, half as many row hand-offs)
+#ifndef GP_EROWS
+#define GP_EROWS 1
+#endif
+constexpr int EROWS = GP_EROWS;
+static_assert(FY % EROWS == 0 && (EROWS == 1 || EROWS == 2), "one or two footprint rows per Eulerian warp");
+constexpr int NEW = FY / EROWS;           // Eulerian warps, one per EROWS footprint rows
 constexpr int NDW = GP_NDW;               // Lagrangian / producer warps
 constexpr int NTE = NEW * 32, NTD = NDW * 32, NT = NTE + NTD;
 constexpr int DROWS = TYO / NDW;          // output rows per Lagrangian warp
@@ -548,9 +555,10 @@ constexpr int OY_LO = 0, OY_OWN = 8, OY_UP = 16, OP_LO = 8 * FY, OP_OWN = 8 + 8 
 static_assert(offsetof(BlockTab, landed) == 0 && offsetof(BlockTab, ufull) == 8 * NS, "ring barriers are addressed from the table base");
 static_assert(offsetof(BlockTab, prdy) == offsetof(BlockTab, yrdy) + 8 * FY, "row barriers are addressed from yrdy");
 
-__device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b, const BlockTab* T) {
+// row: footprint row of the thread (the q-th row of warp w is EROWS * w + q); the hand-off barriers are per warp
+__device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b, const BlockTab* T, int row) {
     Foot f;
-    f.tx = threadIdx.x & 31; f.ty = threadIdx.x >> 5; f.t = f.ty * FX + f.tx;
+    f.tx = threadIdx.x & 31; f.ty = row; f.t = f.ty * FX + f.tx;
     f.xv = b.x0 - 2 + f.tx; f.yv = b.y0 - 2 + f.ty;
     f.nxny = (size_t)g.nx * g.ny;
     f.base = (size_t)map_safe(f.xv, g.nx, g.bcx) + (size_t)g.nx * map_safe(f.yv, g.ny, g.bcy);
@@ -567,7 +575,7 @@ __device__ __forceinline__ Foot make_foot(const Geo& g, const Blk& b, const Bloc
     }
     f.fix = f.fix && f.star_row && f.tx >= 1 && f.tx <= FX - 2;
     f.tabbar = smem_u32(T);
-    f.rowbar = smem_u32(&T->yrdy[0]) + 8 * (f.ty - 1);
+    f.rowbar = smem_u32(&T->yrdy[0]) + 8 * ((int)(threadIdx.x >> 5) - 1);
     return f;
 }
 
@@ -764,6 +772,36 @@ struct GasShared {
     double *rp, *vx, *vy, *phi, *fy, *fyv, *ring, *tz;
 };
 
+// Prologue of one Eulerian cell column: primitives of plane z0-2, then plane z0-1 with the z face between them;
+// publishes the primitives of plane z0-1.
+__device__ __forceinline__ GasCarry gas_prologue(const FusedArgs<NFG>& a, const Geo& g, const Blk& b, const Foot& f, const GasShared& S,
+                                                 double th, double gm1) {
+    GasCarry c;
+    const int t = f.t;
+    int zm = map_safe(b.z0 - 2, g.nz, g.bcz);
+    size_t off = f.base + (size_t)zm * f.nxny;
+    constexpr int ES = OD ? BSTR : 1;        // the energy is paired with rho*eps under GP_OD
+    double rho = a.U[0][BSTR * off], mx = a.U[1][BSTR * off], my = a.U[2][BSTR * off], mz = a.U[3][BSTR * off], E = a.U[4][ES * off];
+    double ir = frcp(rho);
+    const double vz_a = mz * ir;
+    // same expression as the main loop, so that a 1-D problem stays bitwise 1-D across the chunk edge
+    const double p_a = OD ? gm1 * a.U[IEPS][BSTR * off] : gm1 * (E - 0.5 * fma(mx, mx * ir, fma(my, my * ir, mz * vz_a)));
+    const double rho_a = rho;
+    zm = map_safe(b.z0 - 1, g.nz, g.bcz);
+    off = f.base + (size_t)zm * f.nxny;
+    rho = a.U[0][BSTR * off]; mx = a.U[1][BSTR * off]; my = a.U[2][BSTR * off]; mz = a.U[3][BSTR * off]; E = a.U[4][ES * off];
+    ir = frcp(rho);
+    c.rho = rho; c.ir = ir; c.vx = mx * ir; c.vy = my * ir; c.vz = mz * ir;
+    c.eps = OD ? a.U[IEPS][BSTR * off] : 0.0;
+    c.p = OD ? gm1 * c.eps : gm1 * (E - 0.5 * fma(mx, c.vx, fma(my, c.vy, mz * c.vz)));
+    double Pz, PVz, Vz;
+    gas_face(a.gamma, rho_a, vz_a, p_a, c.rho, c.vz, c.p, Pz, PVz, Vz);
+    c.adv = -Vz;
+    c.amx = mx; c.amy = my; c.amz = fma(0.5 * th, Pz, mz); c.aE = fma(0.25 * th, PVz, E);
+    sts2(S.rp + 2 * t, c.rho, c.p); S.vx[t] = c.vx; S.vy[t] = c.vy;
+    return c;
+}
+
 template <bool ST>
 __device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, const Blk& b, const Foot& f, const GasShared& S,
                                          GasCarry& c, int j, double tau, double th, double inv2h) {
@@ -909,6 +947,150 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, c
     if (f.tx == 0) mbar_arrive_at<8 * NS>(slotbar);   // this row's U*(j) is complete
 }
 
+#if GP_EROWS == 2
+// Two footprint rows per thread (rows 2w and 2w+1 of Eulerian warp w): the y face between them is solved once and
+// stays in registers, the face above the upper row goes to the warp above through shared memory as before.  Plain
+// scheme only (no GP_OVERDET).  Publishes the primitives of the next plane before the z face solves.
+template <bool ST>
+__device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, const Blk& b, const Foot (&f)[2], const GasShared& S,
+                                          GasCarry (&c)[2], int j, double tau, double th, double inv2h) {
+    static_assert(!OD, "two rows per thread: plain scheme only");
+    const Geo& g = a.g;
+    const int w = threadIdx.x >> 5;
+    const int t0 = f[0].t, t1 = f[1].t, tx = f[0].tx;
+    const double gamma = a.gamma, gm1 = a.gamma - 1.0;
+    const double th2 = 0.5 * th, th4 = 0.25 * th;
+    const bool zout = g.bcz == GP_BC_OUTFLOW;
+    const bool top_copy = !ST && zout && j == g.nz;
+    const bool bot_dup = !ST && zout && j == 0;
+    const bool do_out = ST || j - 1 >= b.z0;
+    const int it = j - (b.z0 - 1);
+    const double* ph0 = S.phi + pslot(it + 1) * PL;
+    const unsigned rowbar = f[0].rowbar;
+    if (it > 0 && w < NEW - 1) mbar_wait_at<OP_UP>(rowbar, (it - 1) & 1);   // primitives of plane j of the warp above are published
+
+    // B: the y face between the two rows, the y face above the upper row, the x faces of both rows
+    const bool s0 = f[0].star_row, s1 = f[1].star_row;      // warp 0: row 0 is halo; last warp: row 1 is halo
+    double Pym, PVym, Vym, Pyh = 0.0, PVyh = 0.0, Vyh, gy0 = 0.0, gy1 = 0.0;
+    gas_face(gamma, c[0].rho, c[0].vy, c[0].p, c[1].rho, c[1].vy, c[1].p, Pym, PVym, Vym);
+    {
+        const int e0 = tx < FX - 1 ? t0 + 1 : t0, e1 = e0 + FX, w0 = tx > 0 ? t0 - 1 : t0, w1 = w0 + FX;
+        if (s1) {
+            const double2 ry = lds2(S.rp + 2 * (t1 + FX)), rx = lds2(S.rp + 2 * e1);
+            double Pxh, PVxh, Vxh;
+            gas_face(gamma, c[1].rho, c[1].vy, c[1].p, ry.x, S.vy[t1 + FX], ry.y, Pyh, PVyh, Vyh);
+            gas_face(gamma, c[1].rho, c[1].vx, c[1].p, rx.x, S.vx[e1], rx.y, Pxh, PVxh, Vxh);
+            sts2(S.fy + 2 * t1, Pyh, PVyh);
+            const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1), PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
+            const double gx = (ph0[e1] - ph0[w1]) * inv2h;
+            gy1 = (ph0[t1 + FX] - ph0[t0]) * inv2h;
+            const double trg = tau * c[1].rho * gx, mx = c[1].rho * c[1].vx;
+            c[1].amx = c[1].amx - th2 * (Pxh - Pxl) - trg;
+            c[1].aE = c[1].aE - th4 * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
+        }
+        if (s0) {
+            const double2 rx = lds2(S.rp + 2 * e0);
+            double Pxh, PVxh, Vxh;
+            gas_face(gamma, c[0].rho, c[0].vx, c[0].p, rx.x, S.vx[e0], rx.y, Pxh, PVxh, Vxh);
+            const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1), PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
+            const double gx = (ph0[e0] - ph0[w0]) * inv2h;
+            gy0 = (ph0[t1] - ph0[t0 - FX]) * inv2h;
+            const double trg = tau * c[0].rho * gx, mx = c[0].rho * c[0].vx;
+            c[0].amx = c[0].amx - th2 * (Pxh - Pxl) - trg;
+            c[0].aE = c[0].aE - th4 * (PVxh - PVxl) - fma(-0.5 * tau, trg, tau * mx) * gx;
+        }
+    }
+    row_arrive_at<OY_OWN>(rowbar);                                    // y fluxes above this warp's upper row are written
+    if (w > 0) mbar_wait_at<OY_LO>(rowbar, it & 1);                 // ... and those above the warp below
+
+    // C: y-flux differences
+    if (s1) {
+        const double trg = tau * c[1].rho * gy1, my = c[1].rho * c[1].vy;
+        c[1].amy = c[1].amy - th2 * (Pyh - Pym) - trg;
+        c[1].aE = c[1].aE - th4 * (PVyh - PVym) - fma(-0.5 * tau, trg, tau * my) * gy1;
+    }
+    if (s0) {
+        const double2 lo = lds2(S.fy + 2 * (t0 - FX));
+        const double trg = tau * c[0].rho * gy0, my = c[0].rho * c[0].vy;
+        c[0].amy = c[0].amy - th2 * (Pym - lo.x) - trg;
+        c[0].aE = c[0].aE - th4 * (PVym - lo.y) - fma(-0.5 * tau, trg, tau * my) * gy0;
+    }
+
+    // E: plane j+1 has arrived in ring slot `it`
+    double* rs = S.ring + rslot(it) * GasTraits::SLOT;
+    const unsigned slotbar = f[0].tabbar + 8 * rslot(it);
+    mbar_wait_at<0>(slotbar, rpar(it));
+    double rho_n[2], mx_n[2], my_n[2], mz_n[2], E_n[2], ir_n[2], vx_n[2], vy_n[2], vz_n[2], p_n[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const int t = f[q].t;
+        const double2 a0 = lds2(rs + 2 * t), a1 = lds2(rs + PP + 2 * t);
+        E_n[q] = rs[2 * PP + t];
+        rho_n[q] = a0.x; mx_n[q] = a0.y; my_n[q] = a1.x; mz_n[q] = a1.y;
+        ir_n[q] = frcp(rho_n[q]);
+        vx_n[q] = mx_n[q] * ir_n[q]; vy_n[q] = my_n[q] * ir_n[q]; vz_n[q] = mz_n[q] * ir_n[q];
+        p_n[q] = gm1 * (E_n[q] - 0.5 * fma(mx_n[q], vx_n[q], fma(my_n[q], vy_n[q], mz_n[q] * vz_n[q])));
+        sts2(S.rp + 2 * t, rho_n[q], p_n[q]); S.vx[t] = vx_n[q]; S.vy[t] = vy_n[q];
+    }
+    row_arrive_at<OP_OWN>(rowbar);                                    // primitives of plane j+1 of both rows are published
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const int t = f[q].t;
+        GasCarry& cq = c[q];
+        double Pz = 0.0, PVz = 0.0, Vz = 0.0;
+        if (f[q].star_row) {
+            gas_face(gamma, cq.rho, cq.vz, cq.p, rho_n[q], vz_n[q], p_n[q], Pz, PVz, Vz);
+            double wx, wy, wz, Es, dens;
+            if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
+                const double* rq = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
+                const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
+                dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y; Es = rq[2 * PP + t];
+            } else {
+                const double gz = (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h;
+                const double trg = tau * cq.rho * gz;
+                const double mz = cq.rho * cq.vz;
+                const double mzs = cq.amz - th2 * Pz - trg;
+                Es = cq.aE - th4 * PVz - fma(-0.5 * tau, trg, tau * mz) * gz;
+                dens = cq.rho; wx = cq.amx * cq.ir; wy = cq.amy * cq.ir; wz = mzs * cq.ir;
+            }
+            sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy); rs[2 * PP + t] = Es;
+            if (bot_dup) {                        // outflow: U*(-1) := U*(0)
+                double* rg = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
+                sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy); rg[2 * PP + t] = Es;
+            }
+            if (do_out) sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(cq.wxm, cq.wx0, wx), sum3(cq.wym, cq.wy0, wy));
+            cq.wxm = bot_dup ? wx : cq.wx0; cq.wym = bot_dup ? wy : cq.wy0;
+            cq.wx0 = wx; cq.wy0 = wy;
+        }
+        cq.amx = mx_n[q]; cq.amy = my_n[q]; cq.amz = fma(th2, Pz, mz_n[q]); cq.aE = fma(th4, PVz, E_n[q]);
+        cq.rho = rho_n[q]; cq.ir = ir_n[q]; cq.vx = vx_n[q]; cq.vy = vy_n[q]; cq.vz = vz_n[q]; cq.p = p_n[q];
+    }
+
+    if (b.block_fix) {
+        group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
+#pragma unroll
+        for (int q = 0; q < 2; ++q)
+            if (f[q].fix) {
+                const int t = f[q].t, src = f[q].fix_src;
+#pragma unroll
+                for (int P = 0; P < GasTraits::NPAIR; ++P) {
+                    const double2 v = lds2(rs + P * PP + 2 * src);
+                    sts2(rs + P * PP + 2 * t, v.x, v.y);
+                    if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + P * PP + 2 * t, v.x, v.y);
+                }
+                const double e = rs[2 * PP + src];
+                rs[2 * PP + t] = e;
+                if (bot_dup) S.ring[rslot(it + NS - 1) * GasTraits::SLOT + 2 * PP + t] = e;
+                const double2 v = lds2(S.tz + (it % NTZ) * PP + 2 * src);
+                sts2(S.tz + (it % NTZ) * PP + 2 * t, v.x, v.y);
+            }
+        group_sync(&T->esync, 0);
+    }
+    __syncwarp();
+    if (tx == 0) mbar_arrive_at<8 * NS>(slotbar);   // this warp's U*(j) is complete
+}
+#endif  // GP_EROWS == 2
+
 __global__ void __launch_bounds__(NT, 1)
 k_fused_gas(const __grid_constant__ FusedArgs<NFG> a) {
     extern __shared__ __align__(128) unsigned char smraw[];
@@ -948,39 +1130,27 @@ k_fused_gas(const __grid_constant__ FusedArgs<NFG> a) {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
 #endif
-        const Foot f = make_foot(g, b, T);
-        const int t = f.t;
-        GasCarry c;
-        {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
-            int zm = map_safe(b.z0 - 2, g.nz, g.bcz);
-            size_t off = f.base + (size_t)zm * f.nxny;
-            constexpr int ES = OD ? BSTR : 1;        // the energy is paired with rho*eps under GP_OD
-            double rho = a.U[0][BSTR * off], mx = a.U[1][BSTR * off], my = a.U[2][BSTR * off], mz = a.U[3][BSTR * off], E = a.U[4][ES * off];
-            double ir = frcp(rho);
-            const double vz_a = mz * ir;
-            // same expression as the main loop, so that a 1-D problem stays bitwise 1-D across the chunk edge
-            const double p_a = OD ? gm1 * a.U[IEPS][BSTR * off] : gm1 * (E - 0.5 * fma(mx, mx * ir, fma(my, my * ir, mz * vz_a)));
-            const double rho_a = rho;
-            zm = map_safe(b.z0 - 1, g.nz, g.bcz);
-            off = f.base + (size_t)zm * f.nxny;
-            rho = a.U[0][BSTR * off]; mx = a.U[1][BSTR * off]; my = a.U[2][BSTR * off]; mz = a.U[3][BSTR * off]; E = a.U[4][ES * off];
-            ir = frcp(rho);
-            c.rho = rho; c.ir = ir; c.vx = mx * ir; c.vy = my * ir; c.vz = mz * ir;
-            c.eps = OD ? a.U[IEPS][BSTR * off] : 0.0;
-            c.p = OD ? gm1 * c.eps : gm1 * (E - 0.5 * fma(mx, c.vx, fma(my, c.vy, mz * c.vz)));
-            double Pz, PVz, Vz;
-            gas_face(a.gamma, rho_a, vz_a, p_a, c.rho, c.vz, c.p, Pz, PVz, Vz);
-            c.adv = -Vz;
-            c.amx = mx; c.amy = my; c.amz = fma(0.5 * th, Pz, mz); c.aE = fma(0.25 * th, PVz, E);
-            sts2(S.rp + 2 * t, c.rho, c.p); S.vx[t] = c.vx; S.vy[t] = c.vy;
-        }
+#if GP_EROWS == 2
+        const int w = threadIdx.x >> 5;
+        const Foot f[2] = {make_foot(g, b, T, 2 * w), make_foot(g, b, T, 2 * w + 1)};
+        GasCarry c[2] = {gas_prologue(a, g, b, f[0], S, th, gm1), gas_prologue(a, g, b, f[1], S, th, gm1)};
+#else
+        const Foot f = make_foot(g, b, T, threadIdx.x >> 5);
+        GasCarry c = gas_prologue(a, g, b, f, S, th, gm1);
+#endif
         mbar_wait(&T->pro, 0);
         group_sync(&T->esync, 0);
 
         int j = b.z0 - 1;
+#if GP_EROWS == 2
+        for (; j <= b.z0 && j <= b.z1; ++j) gas_iter2<false>(a, T, b, f, S, c, j, tau, th, inv2h);
+        for (; j <= b.z1 - 1; ++j) gas_iter2<true>(a, T, b, f, S, c, j, tau, th, inv2h);
+        for (; j <= b.z1; ++j) gas_iter2<false>(a, T, b, f, S, c, j, tau, th, inv2h);
+#else
         for (; j <= b.z0 && j <= b.z1; ++j) gas_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1 - 1; ++j) gas_iter<true>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1; ++j) gas_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
+#endif
     }
     block_max_commit(smax, bad, a.smax_bits, a.flag, S.rp, kap, a.kappa);
 }
@@ -1381,7 +1551,7 @@ k_fused_bme(const __grid_constant__ FusedArgs<NFB> a) {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
 #endif
-        const Foot f = make_foot(g, b, T);
+        const Foot f = make_foot(g, b, T, threadIdx.x >> 5);
         const int t = f.t;
         BmeCarry c;
         {   // prologue: primitives of plane z0-2, then plane z0-1 with the z face between them
