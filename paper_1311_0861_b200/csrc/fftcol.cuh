@@ -106,7 +106,7 @@ struct ZExchange {
 // complex products (4 loads less and 16 fp64 operations more per butterfly; the products of unit-modulus numbers lose
 // 2-3 ulp, far inside the 1e-11 bar of the potential)
 #ifndef GP_TW_DERIVE
-#define GP_TW_DERIVE 0
+#define GP_TW_DERIVE 1
 #endif
 
 template <int P, int s, bool INV>
@@ -120,7 +120,9 @@ __device__ __forceinline__ void zstage(double2* v, const double2* __restrict__ t
         double2 w[8];
         if (Q > 1) {
             if (R == 8) {
-                w[1] = tw[o * st]; w[2] = tw[o * 2 * st]; w[4] = tw[o * 4 * st];
+                w[1] = tw[o * st];
+                if (GP_TW_DERIVE >= 2) { w[2] = cmul<false>(w[1], w[1]); w[4] = cmul<false>(w[2], w[2]); }   // one load only
+                else { w[2] = tw[o * 2 * st]; w[4] = tw[o * 4 * st]; }
                 w[3] = cmul<false>(w[1], w[2]); w[5] = cmul<false>(w[1], w[4]); w[6] = cmul<false>(w[2], w[4]);
                 w[7] = cmul<false>(w[3], w[4]);
             } else {
