@@ -7,7 +7,9 @@
 // that work on different planes at the same time, so that the shared-memory-heavy Lagrangian stage
 // of one plane overlaps the fp64-heavy Eulerian stage of a later one:
 //
-//   * FY Eulerian warps ("E", one per footprint row, thread = one cell column).  Per plane j:
+//   * Eulerian warps ("E"; GP_EROWS = 1: one per footprint row, thread = one cell column; GP_EROWS = 2, the gas
+//     kernel: one per two adjacent rows, thread = two cells, the y face between them solved once in registers).
+//     Per plane j:
 //       B  x and y faces of plane j, each computed ONCE (hi face per thread; the lo face comes
 //          from the lane to the left by warp shuffle and from the row below through shared memory);
 //       C  flux differences and the gravity source into U*(j), held in registers;
@@ -37,7 +39,7 @@
 // the Poisson mode, so its staging needs no case analysis.
 //
 // Build parameters (set per translation unit by fused_gas.cu, fused_bme.cu and their _od twins): GP_FY, GP_NDW,
-// GP_NS, GP_REG_E / GP_REG_D, GP_OVERDET, GP_TZREG, GP_EARLYPUB, GP_YRECOMP, GP_WAIT_MODE; the measured effect of
+// GP_NS, GP_EROWS, GP_REG_E / GP_REG_D, GP_OVERDET, GP_TZREG, GP_EARLYPUB, GP_YRECOMP, GP_WAIT_MODE; the measured effect of
 // each is recorded in DESIGN.md section 8.
 #include <cuda.h>
 
