@@ -22,6 +22,10 @@
 #define GP_GASOD_TZREG 0
 #endif
 #define GP_TZREG GP_GASOD_TZREG
+#ifndef GP_GASOD_EROWS
+#define GP_GASOD_EROWS 1
+#endif
+#define GP_EROWS GP_GASOD_EROWS
 #define GP_FUSED_NS fgasod
 #define GP_FUSED_GAS 1
 #include "fused_impl.cuh"

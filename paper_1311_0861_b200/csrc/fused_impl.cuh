@@ -954,12 +954,11 @@ __device__ __forceinline__ void gas_iter(const FusedArgs<NFG>& a, BlockTab* T, c
 
 #if GP_EROWS == 2
 // Two footprint rows per thread (rows 2w and 2w+1 of Eulerian warp w): the y face between them is solved once and
-// stays in registers, the face above the upper row goes to the warp above through shared memory as before.  Plain
-// scheme only (no GP_OVERDET).  Publishes the primitives of the next plane before the z face solves.
+// stays in registers, the face above the upper row goes to the warp above through shared memory as before.
+// Publishes the primitives of the next plane before the z face solves.
 template <bool ST>
 __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, const Blk& b, const Foot (&f)[2], const GasShared& S,
                                           GasCarry (&c)[2], int j, double tau, double th, double inv2h) {
-    static_assert(!OD, "two rows per thread: plain scheme only");
     const Geo& g = a.g;
     const int w = threadIdx.x >> 5;
     const int t0 = f[0].t, t1 = f[1].t, tx = f[0].tx;
@@ -976,7 +975,7 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
 
     // B: the y face between the two rows, the y face above the upper row, the x faces of both rows
     const bool s0 = f[0].star_row, s1 = f[1].star_row;      // warp 0: row 0 is halo; last warp: row 1 is halo
-    double Pym, PVym, Vym, Pyh = 0.0, PVyh = 0.0, Vyh, gy0 = 0.0, gy1 = 0.0;
+    double Pym, PVym, Vym, Pyh = 0.0, PVyh = 0.0, Vyh = 0.0, gy0 = 0.0, gy1 = 0.0;
     gas_face(gamma, c[0].rho, c[0].vy, c[0].p, c[1].rho, c[1].vy, c[1].p, Pym, PVym, Vym);
     {
         const int e0 = tx < FX - 1 ? t0 + 1 : t0, e1 = e0 + FX, w0 = tx > 0 ? t0 - 1 : t0, w1 = w0 + FX;
@@ -986,6 +985,7 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
             gas_face(gamma, c[1].rho, c[1].vy, c[1].p, ry.x, S.vy[t1 + FX], ry.y, Pyh, PVyh, Vyh);
             gas_face(gamma, c[1].rho, c[1].vx, c[1].p, rx.x, S.vx[e1], rx.y, Pxh, PVxh, Vxh);
             sts2(S.fy + 2 * t1, Pyh, PVyh);
+            if (OD) { S.fyv[t1] = Vyh; c[1].adv += Vxh - __shfl_up_sync(0xffffffffu, Vxh, 1); }
             const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1), PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
             const double gx = (ph0[e1] - ph0[w1]) * inv2h;
             gy1 = (ph0[t1 + FX] - ph0[t0]) * inv2h;
@@ -997,6 +997,7 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
             const double2 rx = lds2(S.rp + 2 * e0);
             double Pxh, PVxh, Vxh;
             gas_face(gamma, c[0].rho, c[0].vx, c[0].p, rx.x, S.vx[e0], rx.y, Pxh, PVxh, Vxh);
+            if (OD) c[0].adv += Vxh - __shfl_up_sync(0xffffffffu, Vxh, 1);
             const double Pxl = __shfl_up_sync(0xffffffffu, Pxh, 1), PVxl = __shfl_up_sync(0xffffffffu, PVxh, 1);
             const double gx = (ph0[e0] - ph0[w0]) * inv2h;
             gy0 = (ph0[t1] - ph0[t0 - FX]) * inv2h;
@@ -1013,28 +1014,32 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
         const double trg = tau * c[1].rho * gy1, my = c[1].rho * c[1].vy;
         c[1].amy = c[1].amy - th2 * (Pyh - Pym) - trg;
         c[1].aE = c[1].aE - th4 * (PVyh - PVym) - fma(-0.5 * tau, trg, tau * my) * gy1;
+        if (OD) c[1].adv += Vyh - Vym;
     }
     if (s0) {
         const double2 lo = lds2(S.fy + 2 * (t0 - FX));
         const double trg = tau * c[0].rho * gy0, my = c[0].rho * c[0].vy;
         c[0].amy = c[0].amy - th2 * (Pym - lo.x) - trg;
         c[0].aE = c[0].aE - th4 * (PVym - lo.y) - fma(-0.5 * tau, trg, tau * my) * gy0;
+        if (OD) c[0].adv += Vym - S.fyv[t0 - FX];
     }
 
     // E: plane j+1 has arrived in ring slot `it`
     double* rs = S.ring + rslot(it) * GasTraits::SLOT;
     const unsigned slotbar = f[0].tabbar + 8 * rslot(it);
     mbar_wait_at<0>(slotbar, rpar(it));
-    double rho_n[2], mx_n[2], my_n[2], mz_n[2], E_n[2], ir_n[2], vx_n[2], vy_n[2], vz_n[2], p_n[2];
+    double rho_n[2], mx_n[2], my_n[2], mz_n[2], E_n[2], eps_n[2], ir_n[2], vx_n[2], vy_n[2], vz_n[2], p_n[2];
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
         const int t = f[q].t;
         const double2 a0 = lds2(rs + 2 * t), a1 = lds2(rs + PP + 2 * t);
-        E_n[q] = rs[2 * PP + t];
+        if (OD) { const double2 a2 = lds2(rs + 2 * PP + 2 * t); E_n[q] = a2.x; eps_n[q] = a2.y; }
+        else { E_n[q] = rs[2 * PP + t]; eps_n[q] = 0.0; }
         rho_n[q] = a0.x; mx_n[q] = a0.y; my_n[q] = a1.x; mz_n[q] = a1.y;
         ir_n[q] = frcp(rho_n[q]);
         vx_n[q] = mx_n[q] * ir_n[q]; vy_n[q] = my_n[q] * ir_n[q]; vz_n[q] = mz_n[q] * ir_n[q];
-        p_n[q] = gm1 * (E_n[q] - 0.5 * fma(mx_n[q], vx_n[q], fma(my_n[q], vy_n[q], mz_n[q] * vz_n[q])));
+        // GP_OD: the pressure comes from the carried internal energy (4th equation)
+        p_n[q] = OD ? gm1 * eps_n[q] : gm1 * (E_n[q] - 0.5 * fma(mx_n[q], vx_n[q], fma(my_n[q], vy_n[q], mz_n[q] * vz_n[q])));
         sts2(S.rp + 2 * t, rho_n[q], p_n[q]); S.vx[t] = vx_n[q]; S.vy[t] = vy_n[q];
     }
     row_arrive_at<OP_OWN>(rowbar);                                    // primitives of plane j+1 of both rows are published
@@ -1045,11 +1050,13 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
         double Pz = 0.0, PVz = 0.0, Vz = 0.0;
         if (f[q].star_row) {
             gas_face(gamma, cq.rho, cq.vz, cq.p, rho_n[q], vz_n[q], p_n[q], Pz, PVz, Vz);
-            double wx, wy, wz, Es, dens;
+            double wx, wy, wz, Es, dens, epss = 0.0;
             if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
                 const double* rq = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
                 const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
-                dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y; Es = rq[2 * PP + t];
+                dens = q0.x; wz = q0.y; wx = q1.x; wy = q1.y;
+                if (OD) { const double2 q2 = lds2(rq + 2 * PP + 2 * t); Es = q2.x; epss = q2.y; }
+                else Es = rq[2 * PP + t];
             } else {
                 const double gz = (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h;
                 const double trg = tau * cq.rho * gz;
@@ -1057,11 +1064,14 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
                 const double mzs = cq.amz - th2 * Pz - trg;
                 Es = cq.aE - th4 * PVz - fma(-0.5 * tau, trg, tau * mz) * gz;
                 dens = cq.rho; wx = cq.amx * cq.ir; wy = cq.amy * cq.ir; wz = mzs * cq.ir;
+                if (OD) epss = fma(-(th2 * gm1) * cq.eps, cq.adv + Vz, cq.eps);
             }
-            sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy); rs[2 * PP + t] = Es;
+            sts2(rs + 2 * t, dens, wz); sts2(rs + PP + 2 * t, wx, wy);
+            if (OD) sts2(rs + 2 * PP + 2 * t, Es, epss); else rs[2 * PP + t] = Es;
             if (bot_dup) {                        // outflow: U*(-1) := U*(0)
                 double* rg = S.ring + rslot(it + NS - 1) * GasTraits::SLOT;
-                sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy); rg[2 * PP + t] = Es;
+                sts2(rg + 2 * t, dens, wz); sts2(rg + PP + 2 * t, wx, wy);
+                if (OD) sts2(rg + 2 * PP + 2 * t, Es, epss); else rg[2 * PP + t] = Es;
             }
             if (do_out) sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(cq.wxm, cq.wx0, wx), sum3(cq.wym, cq.wy0, wy));
             cq.wxm = bot_dup ? wx : cq.wx0; cq.wym = bot_dup ? wy : cq.wy0;
@@ -1069,6 +1079,7 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
         }
         cq.amx = mx_n[q]; cq.amy = my_n[q]; cq.amz = fma(th2, Pz, mz_n[q]); cq.aE = fma(th4, PVz, E_n[q]);
         cq.rho = rho_n[q]; cq.ir = ir_n[q]; cq.vx = vx_n[q]; cq.vy = vy_n[q]; cq.vz = vz_n[q]; cq.p = p_n[q];
+        if (OD) { cq.eps = eps_n[q]; cq.adv = -Vz; }
     }
 
     if (b.block_fix) {
@@ -1083,9 +1094,11 @@ __device__ __forceinline__ void gas_iter2(const FusedArgs<NFG>& a, BlockTab* T, 
                     sts2(rs + P * PP + 2 * t, v.x, v.y);
                     if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * GasTraits::SLOT + P * PP + 2 * t, v.x, v.y);
                 }
-                const double e = rs[2 * PP + src];
-                rs[2 * PP + t] = e;
-                if (bot_dup) S.ring[rslot(it + NS - 1) * GasTraits::SLOT + 2 * PP + t] = e;
+                if (GasTraits::LAST1) {
+                    const double e = rs[2 * PP + src];
+                    rs[2 * PP + t] = e;
+                    if (bot_dup) S.ring[rslot(it + NS - 1) * GasTraits::SLOT + 2 * PP + t] = e;
+                }
                 const double2 v = lds2(S.tz + (it % NTZ) * PP + 2 * src);
                 sts2(S.tz + (it % NTZ) * PP + 2 * t, v.x, v.y);
             }
