@@ -1148,6 +1148,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NFG> a) {
 #if GP_REG_E
         reg_alloc<GP_REG_E>();
 #endif
+        if ((int)threadIdx.x < NEW * 32) {
 #if GP_EROWS == 2
         const int w = threadIdx.x >> 5;
         const Foot f[2] = {make_foot(g, b, T, 2 * w), make_foot(g, b, T, 2 * w + 1)};
@@ -1169,6 +1170,7 @@ k_fused_gas(const __grid_constant__ FusedArgs<NFG> a) {
         for (; j <= b.z1 - 1; ++j) gas_iter<true>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1; ++j) gas_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
 #endif
+        }   // real Eulerian warps (the padding warps of the register split skip to the reduction)
     }
     block_max_commit(smax, bad, a.smax_bits, a.flag, S.rp, kap, a.kappa);
 }
