@@ -201,6 +201,49 @@ def test_balance_at_a_vacuum_border_keeps_pressure_positive(orc):
     assert o.kappa()[0] <= 1e-14
 
 
+def test_balance_of_the_collisionless_component_by_hand(orc):
+    """G15 by hand on single cells of a STARS context with uniform n, u != 0 and a carried Pi that drifted everywhere:
+    (a) a healthy cell (all three implied Pi_dd > 0): Pi_ij := n E_ij - n u_i u_j, n E_ij untouched; (b), (c), (d) one
+    cell each whose implied Pi_xx, Pi_yy, Pi_zz ALONE is not positive: the carried tensor wins there and all six
+    n E_ij := Pi_ij + n u_i u_j exactly, n, n u and Pi untouched.  kappa_bme is zero afterwards."""
+    N = 4
+    one = np.ones((N, N, N))
+    nn = 2.0 * one
+    u = [0.5 * one, -0.25 * one, 0.75 * one]
+    Pi_implied = [1.0, 0.2, -0.1, 0.8, 0.05, 1.2]          # xx xy xz yy yz zz, what n E_ij will imply
+    o = orc.Oracle(N, N, N, 1.0, W.STARS)
+    st = W._pack_stars(nn, u, [v * one for v in Pi_implied])
+    o.set_state(st)
+    o.od_enable()
+    carried = [0.6, 0.1, 0.02, 0.5, -0.04, 0.9]             # the drifted carried tensor, different in every component
+    for name, v in zip(PN, carried):
+        o.set(name, v * one)
+    E = {e: st[e].copy() for e in EN}
+    nuu = {e: 2.0 * u[i][0, 0, 0] * u[j][0, 0, 0] for e, (i, j) in zip(EN, PAIRS)}
+    bad = {"Exx": (0, 0, 1), "Eyy": (0, 0, 2), "Ezz": (0, 0, 3)}   # one diagonal each: implied Pi_dd = -0.3
+    for e, cell in bad.items():
+        E[e][cell] = nuu[e] - 0.3
+    for e in EN:
+        o.set(e, E[e])
+    o.od_balance()
+    got_E = {e: o.get(e) for e in EN}
+    got_P = {p: o.get(p) for p in PN}
+    # (a) healthy cell: total-energy description wins, nE untouched bit for bit
+    for p, e, v in zip(PN, EN, Pi_implied):
+        assert got_P[p][0, 0, 0] == pytest.approx(v, rel=1e-14, abs=1e-15)
+        assert got_E[e][0, 0, 0] == E[e][0, 0, 0]
+    assert np.array_equal(got_E["Exx"][1:], E["Exx"][1:])
+    # (b), (c), (d): carried tensor wins in the whole cell
+    for cell in bad.values():
+        for p, e, v in zip(PN, EN, carried):
+            assert got_P[p][cell] == v, (cell, p)
+            assert got_E[e][cell] == v + nuu[e], (cell, e)
+    assert np.array_equal(o.get("n"), nn)
+    for k, a in zip(("nux", "nuy", "nuz"), u):
+        assert np.array_equal(o.get(k), nn * a)
+    assert o.kappa()[1] <= 1e-14
+
+
 def test_dispersion_equation_agrees_with_the_energy_tensor_on_smooth_shear(orc):
     """One unbalanced step of a smooth state with all six Pi components and all velocities varying: the Pi_ij carried by
     PAPER.md:65 and the one implied by n E_ij differ by the truncation error only, first order in h."""
