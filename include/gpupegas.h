@@ -131,6 +131,40 @@ int gp_od_balance(gp_ctx* ctx);
 int gp_kappa(gp_ctx* ctx, double* out);
 int gp_od_last_kappa(gp_ctx* ctx, double* out);
 
+/* ---- the correctness check for callers who cannot let the library allocate ----
+ * gp_kappa needs a context, and a context takes device storage of about twice the state (cudaMalloc at first use,
+ * or a region the caller binds).  Some callers have no memory to give and cannot tolerate an allocation: a run
+ * whose grids fill the card, a PyTorch process whose caching allocator already holds the free HBM (a cudaMalloc
+ * from in here then fails, or starves that allocator later), a multi-stream time loop (cudaMalloc / cudaFree stall
+ * the whole device), or a tool that merely holds the fields of some snapshot and wants the two sums.  For them:
+ *
+ * gp_kappa_noalloc: out_device[0] = kappa_gas, out_device[1] = kappa_bme, the sums defined under gp_kappa, of the
+ *   fields the caller passes.  No context; the call never calls cudaMalloc, cudaFree or any allocating library
+ *   routine, and copies nothing.
+ *   n_cells   number of cells, 1 ... GP_KAPPA_NOALLOC_MAX_CELLS (512^3); more: GP_ERR_ARG (a larger grid can be
+ *             summed slab by slab, adding the results).
+ *   h         cell size (> 0); the sums are multiplied by h^3.
+ *   gas       HOST array of 6 DEVICE pointers, each to n_cells contiguous doubles: rho, rho v_x, rho v_y, rho v_z,
+ *             rho E, rho eps; or NULL (kappa_gas = 0).
+ *   stars     HOST array of 16 DEVICE pointers: n, n u_x, n u_y, n u_z, n E_ij (xx xy xz yy yz zz), Pi_ij (same
+ *             order); or NULL (kappa_bme = 0).  Not both NULL.  The fields are only read and stay the caller's.
+ *   out_device  DEVICE pointer to 2 doubles, written by the last kernel of the call.
+ *   cuda_stream a cudaStream_t of the current device (NULL: default stream).  The two kernels are issued on it and
+ *             the call returns without synchronising; the result is ready when work queued behind it runs.
+ *   Scratch: the per-block partial sums sit in a 512 KiB array compiled into the library (one pair of doubles per
+ *   4096 cells, which is where the limit comes from).  Every GPU that has loaded the library holds that array
+ *   until the process ends.  All calls on a GPU share it: calls issued on ONE stream are safe back to back (each
+ *   call rewrites every slot it later reads, so nothing needs to start at zero), but two calls that can overlap on
+ *   the GPU -- different streams without an event between them, or two host threads -- race on it and may both
+ *   return garbage.  The first call on each device looks up the array's device address (which may make the driver
+ *   load the module); make that first call outside any stream capture.  The result is bit-reproducible for given
+ *   inputs; it differs from gp_kappa's only by the rounding of a different summation order.
+ *   Errors: GP_ERR_ARG as above (also a NULL pointer inside gas / stars), GP_ERR_CUDA if the address look-up or a
+ *   launch fails, GP_ERR_UNSUPPORTED for a device ordinal >= 64. */
+#define GP_KAPPA_NOALLOC_MAX_CELLS 134217728
+int gp_kappa_noalloc(size_t n_cells, double h, const double* const* gas, const double* const* stars,
+                     double* out_device, void* cuda_stream);
+
 const char* gp_last_error(void);   /* thread-local static text; never freed by the caller */
 
 /* ---- optional: let the caller (e.g. PyTorch) own the stream and the device memory ---- */

@@ -25,7 +25,9 @@ GAS_FIELDS, STAR_FIELDS = FIELDS[:5], FIELDS[5:15]
 EXPORTS = ["gp_create", "gp_destroy", "gp_set_state", "gp_get_state", "gp_solve_poisson", "gp_max_dt",
            "gp_step", "gp_last_error", "gp_set_stream", "gp_storage_bytes", "gp_bind_storage",
            "gp_synchronize", "gp_launch_counts", "gp_timing_enable", "gp_timing_read", "gp_math_selftest",
-           "gp_fp64_rate_selftest", "gp_od_derive", "gp_od_step", "gp_od_balance", "gp_kappa", "gp_od_last_kappa"]
+           "gp_fp64_rate_selftest", "gp_od_derive", "gp_od_step", "gp_od_balance", "gp_kappa", "gp_od_last_kappa",
+           "gp_kappa_noalloc"]
+KAPPA_NOALLOC_MAX_CELLS = 134217728      # GP_KAPPA_NOALLOC_MAX_CELLS
 
 
 class gp_grid(C.Structure):
@@ -80,6 +82,7 @@ def lib():
         L.gp_od_balance.argtypes = [vp]
         L.gp_kappa.argtypes = [vp, dp]
         L.gp_od_last_kappa.argtypes = [vp, dp]
+        L.gp_kappa_noalloc.argtypes = [C.c_size_t, C.c_double, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -98,6 +101,27 @@ def fp64_rate_selftest():
     rate, ms = C.c_double(0.0), C.c_double(0.0)
     _chk(lib().gp_fp64_rate_selftest(C.byref(rate), C.byref(ms)), "gp_fp64_rate_selftest")
     return rate.value, ms.value
+
+
+def kappa_noalloc(h, gas=None, stars=None, out=None, stream=None):
+    """gp_kappa_noalloc: (kappa_gas, kappa_bme) of fields the caller already holds on the device, for programs that
+    cannot let the library allocate (all HBM already spoken for by the caller's own pool, or a loop that must not
+    stall on cudaMalloc).  `gas`: 6 float64 CUDA tensors (rho, mx, my, mz, E, eps), `stars`: 16 (n, nu*, E**, P**),
+    all of the same number of elements, contiguous; `out`: a float64 CUDA tensor of 2 elements (the caller's too:
+    nothing is allocated here), returned.  Asynchronous on `stream` (default: torch's current stream).  The
+    library's one fixed scratch array is shared by all calls on a GPU, so do not let two calls overlap."""
+    import torch
+    groups = [g for g in (gas, stars) if g is not None]
+    assert groups and out is not None and out.is_cuda and out.dtype == torch.float64 and out.numel() == 2
+    assert (gas is None or len(gas) == 6) and (stars is None or len(stars) == 16)
+    n = groups[0][0].numel()
+    for g in groups:
+        for t in g:
+            assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n
+    as_ptrs = lambda g: None if g is None else (C.c_void_p * len(g))(*[t.data_ptr() for t in g])
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _chk(lib().gp_kappa_noalloc(n, h, as_ptrs(gas), as_ptrs(stars), out.data_ptr(), st.cuda_stream), "gp_kappa_noalloc")
+    return out
 
 
 def _chk(code, what):

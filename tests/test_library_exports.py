@@ -78,6 +78,8 @@ def test_binding_constants_match_the_header():
     for py_name, c_name in zip(order, names):
         assert B.FIELD_ID[py_name] == values["GP_" + c_name], (py_name, c_name)
     assert (B.GP_GAS, B.GP_STARS, B.GP_OD) == (values["GP_GAS"], values["GP_STARS"], values["GP_OD"])
+    define = re.search(r"#define\s+GP_KAPPA_NOALLOC_MAX_CELLS\s+(\d+)", text)
+    assert define and int(define.group(1)) == B.KAPPA_NOALLOC_MAX_CELLS == 512 ** 3
     assert (B.GP_ERR_STATE, B.GP_ERR_UNSUPPORTED) == (values["GP_ERR_STATE"], values["GP_ERR_UNSUPPORTED"])
     assert (B.GP_POISSON_PERIODIC, B.GP_POISSON_ISOLATED, B.GP_BC_OUTFLOW) == (
         values["GP_POISSON_PERIODIC"], values["GP_POISSON_ISOLATED"], values["GP_BC_OUTFLOW"])
