@@ -436,6 +436,10 @@ def main():
         return
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: --gpus N starts the N replica ranks itself (rank 0 prints the line with n_gpus = N)
+        from paper_1311_0861_b200 import distrib
+        sys.exit(distrib.launch_replicas(args.gpus, [sys.executable, os.path.abspath(__file__)] + sys.argv[1:]))
     else:
         run_gpu(args)
 

@@ -14,6 +14,37 @@ def env_world():
             int(os.environ.get("WORLD_SIZE", "1")))
 
 
+def free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_replicas(n, argv, timeout=None):
+    """Start `n` copies of the command `argv`, one per GPU, the way torchrun would (RANK = LOCAL_RANK = 0..n-1,
+    WORLD_SIZE = n, MASTER_ADDR 127.0.0.1, a free MASTER_PORT), and wait for them.  Rank 0 inherits this process's
+    stdout (it prints the one JSON line); the other ranks' stdout is dropped, every rank's stderr is inherited.
+    Returns the largest exit code.  This is what `python bench.py --gpus N` does when it is not already running
+    under torchrun; processes are started and stopped by handle, never by name."""
+    import subprocess
+    port = free_port()
+    procs = []
+    for rank in range(n):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(n),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen(list(argv), env=env, stdout=None if rank == 0 else subprocess.DEVNULL))
+    rc = 0
+    try:
+        for p in procs:
+            rc = max(rc, abs(p.wait(timeout=timeout)))
+    finally:
+        for p in procs:
+            if p.poll() is None:
+                p.kill()
+    return rc
+
+
 def init(backend, device=None):
     import torch.distributed as dist
     rank, _, world = env_world()

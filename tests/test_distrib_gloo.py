@@ -64,3 +64,42 @@ def test_single_process_is_a_no_op():
     distrib.barrier()
     assert distrib.max_over_ranks(3.5) == 3.5
     assert distrib.aggregate_throughput(10, 2, 4.0, 1) == 10 * 2 / 4.0e-3
+
+
+LAUNCHED = textwrap.dedent("""
+    import json, os, sys
+    sys.path.insert(0, {root!r})
+    from paper_1311_0861_b200 import distrib
+    rank, local_rank, world = distrib.env_world()
+    distrib.init("gloo")
+    distrib.barrier()
+    ms = distrib.max_over_ranks(7.0 + rank)
+    distrib.barrier()
+    distrib.shutdown()
+    print(json.dumps({{"rank": rank, "local_rank": local_rank, "n_gpus": world, "ms": ms}}))   # every rank prints
+""")
+
+
+def test_launcher_starts_n_ranks_and_only_rank_0_reaches_stdout(tmp_path):
+    """`bench.py --gpus N` outside torchrun: distrib.launch_replicas starts the N ranks itself (CPU stub, gloo)."""
+    import json
+    worker = tmp_path / "stub.py"
+    worker.write_text(LAUNCHED.format(root=ROOT))
+    driver = tmp_path / "driver.py"
+    driver.write_text(textwrap.dedent(f"""
+        import sys
+        sys.path.insert(0, {ROOT!r})
+        from paper_1311_0861_b200 import distrib
+        sys.exit(distrib.launch_replicas(3, [sys.executable, {str(worker)!r}], timeout=120))
+    """))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, str(driver)], env=env, capture_output=True, text=True, timeout=180)
+    assert r.returncode == 0, r.stderr
+    lines = [json.loads(x) for x in r.stdout.strip().splitlines()]
+    assert lines == [{"rank": 0, "local_rank": 0, "n_gpus": 3, "ms": 9.0}]      # one line, rank 0's, max over 3 ranks
+
+
+def test_bench_gpus_flag_goes_through_the_launcher():
+    """bench.py hands --gpus N > 1 to the launcher unless torchrun's WORLD_SIZE is already set."""
+    text = open(os.path.join(ROOT, "bench.py")).read()
+    assert 'args.gpus > 1 and "WORLD_SIZE" not in os.environ' in text and "launch_replicas(args.gpus" in text
