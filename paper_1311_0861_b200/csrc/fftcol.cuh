@@ -102,12 +102,9 @@ struct ZExchange {
     }
 };
 
-// GP_TW_DERIVE: a radix-8 stage loads the twiddles w, w^2, w^4 of its butterfly and forms w^3, w^5, w^6, w^7 by
+// A radix-8 stage loads the twiddles w, w^2, w^4 of its butterfly and forms w^3, w^5, w^6, w^7 by
 // complex products (4 loads less and 16 fp64 operations more per butterfly; the products of unit-modulus numbers lose
 // 2-3 ulp, far inside the 1e-11 bar of the potential)
-#ifndef GP_TW_DERIVE
-#define GP_TW_DERIVE 1
-#endif
 
 template <int P, int s, bool INV>
 __device__ __forceinline__ void zstage(double2* v, const double2* __restrict__ tw, int t) {
@@ -116,13 +113,11 @@ __device__ __forceinline__ void zstage(double2* v, const double2* __restrict__ t
 #pragma unroll
     for (int b = 0; b < 8 / R; ++b) {
         const int o = (t + T * b) % Q;
-#if GP_TW_DERIVE
         double2 w[8];
         if (Q > 1) {
             if (R == 8) {
                 w[1] = tw[o * st];
-                if (GP_TW_DERIVE >= 2) { w[2] = cmul<false>(w[1], w[1]); w[4] = cmul<false>(w[2], w[2]); }   // one load only
-                else { w[2] = tw[o * 2 * st]; w[4] = tw[o * 4 * st]; }
+                w[2] = tw[o * 2 * st]; w[4] = tw[o * 4 * st];
                 w[3] = cmul<false>(w[1], w[2]); w[5] = cmul<false>(w[1], w[4]); w[6] = cmul<false>(w[2], w[4]);
                 w[7] = cmul<false>(w[3], w[4]);
             } else {
@@ -131,9 +126,6 @@ __device__ __forceinline__ void zstage(double2* v, const double2* __restrict__ t
             }
         }
 #define GP_TWIDDLE(m) w[m]
-#else
-#define GP_TWIDDLE(m) tw[o * (m) * st]
-#endif
         if (INV && Q > 1) {
 #pragma unroll
             for (int m = 1; m < R; ++m) v[b * R + m] = cmul<true>(v[b * R + m], GP_TWIDDLE(m));

@@ -18,15 +18,6 @@
 #define GP_BME_TZREG 0
 #endif
 #define GP_TZREG GP_BME_TZREG
-#ifndef GP_BME_YRECOMP
-#define GP_BME_YRECOMP 0
-#endif
-#define GP_YRECOMP GP_BME_YRECOMP
-// two footprint rows per Eulerian thread (6 Eulerian warps padded to 8 for the register split + 8 Lagrangian warps)
-#ifndef GP_BME_EROWS
-#define GP_BME_EROWS 1
-#endif
-#define GP_EROWS GP_BME_EROWS
 #define GP_FUSED_NS fbme
 #define GP_FUSED_BME 1
 #include "fused_impl.cuh"

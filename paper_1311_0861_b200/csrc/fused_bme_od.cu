@@ -20,10 +20,6 @@
 #define GP_BMEOD_TZREG 0
 #endif
 #define GP_TZREG GP_BMEOD_TZREG
-#ifndef GP_BMEOD_YRECOMP
-#define GP_BMEOD_YRECOMP 0
-#endif
-#define GP_YRECOMP GP_BMEOD_YRECOMP
 #define GP_FUSED_NS fbmeod
 #define GP_FUSED_BME 1
 #include "fused_impl.cuh"

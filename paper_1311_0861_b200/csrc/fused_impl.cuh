@@ -39,7 +39,7 @@
 // the Poisson mode, so its staging needs no case analysis.
 //
 // Build parameters (set per translation unit by fused_gas.cu, fused_bme.cu and their _od twins): GP_FY, GP_NDW,
-// GP_NS, GP_EROWS, GP_REG_E / GP_REG_D, GP_OVERDET, GP_TZREG, GP_EARLYPUB, GP_YRECOMP, GP_WAIT_MODE; the measured effect of
+// GP_NS, GP_EROWS, GP_REG_E / GP_REG_D, GP_OVERDET, GP_TZREG, GP_EARLYPUB; the measured effect of
 // each is recorded in DESIGN.md section 8.
 #include <cuda.h>
 
@@ -93,13 +93,6 @@ constexpr bool OD = GP_OVERDET != 0;
 #define GP_TZREG 0
 #endif
 constexpr bool TZREG = GP_TZREG != 0;
-// GP_YRECOMP (collisionless kernel): every Eulerian row solves BOTH its y faces (the lower one from the primitives of
-// the row below) instead of taking the lower face's fluxes from the row below through shared memory: one face solve
-// more per cell, 88 bytes of exchange and one row hand-off per plane less, three independent solver chains in stage B
-#ifndef GP_YRECOMP
-#define GP_YRECOMP 0
-#endif
-constexpr bool YRECOMP = GP_YRECOMP != 0;
 // GP_EARLYPUB: stage E publishes the primitives of plane j+1 (and releases the rows waiting for them) as soon as they
 // are recovered, before the z face solve and the U* stores, instead of at the end of the stage
 #ifndef GP_EARLYPUB
@@ -226,17 +219,8 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, uns
 // Wait for the phase of given parity of the mbarrier at shared address base + OFF (bytes; an immediate, so that no
 // second address register stays live across the loop).  try_wait suspends the warp for up to the hinted time, so a
 // waiting warp issues a poll only now and then instead of spinning on the issue port of the working warps.
-// GP_WAIT_MODE: 0 = try_wait in a plain loop, 1 = try_wait with a suspend-time hint (ptxas adds NANOSLEEP.SYNCS),
-// 2 = try_wait, then an explicit nanosleep of GP_WAIT_NS before the next try
-#ifndef GP_WAIT_MODE
-#define GP_WAIT_MODE 1
-#endif
-#ifndef GP_WAIT_NS
-#define GP_WAIT_NS 40
-#endif
 template <int OFF = 0>
 __device__ __forceinline__ void mbar_wait_at(unsigned base, unsigned parity) {
-#if GP_WAIT_MODE == 1
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "W_%=:\n\t"
@@ -245,27 +229,6 @@ __device__ __forceinline__ void mbar_wait_at(unsigned base, unsigned parity) {
         "bra W_%=;\n\t"
         "D_%=:\n\t}" ::"r"(base), "r"(parity), "r"(0x989680), "n"(OFF)
         : "memory");
-#elif GP_WAIT_MODE == 0
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "W_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%2], %1;\n\t"
-        "@p bra D_%=;\n\t"
-        "bra W_%=;\n\t"
-        "D_%=:\n\t}" ::"r"(base), "r"(parity), "n"(OFF)
-        : "memory");
-#else
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%2], %1;\n\t"
-        "@p bra D_%=;\n\t"
-        "W_%=:\n\t"
-        "nanosleep.u32 %3;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0+%2], %1;\n\t"
-        "@!p bra W_%=;\n\t"
-        "D_%=:\n\t}" ::"r"(base), "r"(parity), "n"(OFF), "n"(GP_WAIT_NS)
-        : "memory");
-#endif
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) { mbar_wait_at<0>(smem_u32(b), parity); }
 template <int OFF = 0>
@@ -389,11 +352,7 @@ __device__ __forceinline__ void lagrange_add(const double* __restrict__ r, int t
 }
 // does any output lane of the warp take anything from this neighbour?
 __device__ __forceinline__ bool lag_needed(double cq, bool lane_out) {
-#ifdef GP_NO_UPWIND_SKIP
-    return true;
-#else
     return __any_sync(FULL, lane_out && cq != 0.0) != 0;
-#endif
 }
 
 // 32 x the face velocities of one output cell (reading G2) from the z-summed (4 x averaged) w*_x,
@@ -465,9 +424,6 @@ __device__ void build_tab(BlockTab* T, const Geo& g, const PhiPad& phi, const Bl
     // a TMA box neither wraps nor clamps: the footprint must lie inside the grid
     const bool inside = b.x0 - 2 >= 0 && b.x0 - 2 + FX <= g.nx && b.y0 - 2 >= 0 && b.y0 - 2 + FY <= g.ny;
     T->percell = (use_tma && inside) ? 0 : 1;
-#ifdef GP_FORCE_PERCELL
-    T->percell = 1;
-#endif
 }
 
 // Producer (Lagrangian warps): request plane kz of the state into ring slot `dst` (layout above: NPAIR pair
@@ -1333,55 +1289,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
     const int it = j - (b.z0 - 1);
     const double* ph0 = S.phi + pslot(it + 1) * PL;   // Phi(j); Phi(j-1) and Phi(j+1) sit in the slots either side
     if (it > 0 && f.ty < FY - 1) mbar_wait_at<OP_UP>(f.rowbar, (it - 1) & 1);   // primitives of plane j of the row above are published
-    if (YRECOMP && it > 0 && f.ty > 0) mbar_wait_at<OP_LO>(f.rowbar, (it - 1) & 1);   // ... and of the row below
 
-  if (YRECOMP) {
-    // B + C in one basic block: x face (hi; lo from the left lane), BOTH y faces, flux differences, gravity source
-    if (f.star_row) {
-        const int tn = t + FX, ts = t - FX, te = f.tx < FX - 1 ? t + 1 : t;
-        const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
-        const double2 z0 = lds2(S.nu + 2 * ts), z1 = lds2(S.uu + 2 * ts), z2 = lds2(S.py + 2 * ts);
-        const double2 x0 = lds2(S.nu + 2 * te), x1 = lds2(S.uu + 2 * te), x2 = lds2(S.px + 2 * te);
-        const double pxy_n = S.pxy[tn], pxy_s = S.pxy[ts], pxy_e = S.pxy[te];
-        const double ury[3] = {y0.y, y1.x, y1.y}, uly[3] = {z0.y, z1.x, z1.y}, urx[3] = {x0.y, x1.x, x1.y};
-        const double Pcy[3] = {c.Pi[1], c.Pi[3], c.Pi[4]}, Plx[3] = {c.Pi[0], c.Pi[1], c.Pi[2]};
-        const double Pry[3] = {pxy_n, y2.x, y2.y}, Pby[3] = {pxy_s, z2.x, z2.y}, Prx[3] = {x2.x, pxy_e, x2.y};
-        double Py[3], EFy[6], usy[3], Pyl[3], EFyl[6], usyl[3], Px[3], EFx[6], usx[3];
-        bme_face<1>(c.n, c.u, Pcy, y0.x, ury, Pry, Py, EFy, usy);
-        bme_face<1>(z0.x, uly, Pby, c.n, c.u, Pcy, Pyl, EFyl, usyl);
-        bme_face<0>(c.n, c.u, Plx, x0.x, urx, Prx, Px, EFx, usx);
-        if (OD) {
-            double du2[3];
-#pragma unroll
-            for (int q = 0; q < 3; ++q) du2[q] = usx[q] - __shfl_up_sync(0xffffffffu, usx[q], 1);
-            pi_source<0>(c.accP, c.Pi, du2, -th2);
-#pragma unroll
-            for (int q = 0; q < 3; ++q) du2[q] = usy[q] - usyl[q];
-            pi_source<1>(c.accP, c.Pi, du2, -th2);
-        }
-#pragma unroll
-        for (int q = 0; q < 3; ++q) c.acc[q] -= th2 * ((Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1)) + (Py[q] - Pyl[q]));
-#pragma unroll
-        for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th4 * ((EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1)) + (EFy[q] - EFyl[q]));
-        // gravity (reading G5): -tau n g_i and -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
-        const double gr[3] = {(ph0[te] - ph0[f.tx > 0 ? t - 1 : t]) * inv2h, (ph0[tn] - ph0[ts]) * inv2h,
-                              (S.phi[pslot(it + 2) * PL + t] - S.phi[pslot(it) * PL + t]) * inv2h};
-        double uc[3];
-#pragma unroll
-        for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], c.u[d]);
-        const double tn_ = tau * c.n;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) c.acc[d] = fma(-tn_, gr[d], c.acc[d]);
-        c.acc[3] = fma(-tn_, 2.0 * uc[0] * gr[0], c.acc[3]);
-        c.acc[4] = fma(-tn_, fma(uc[0], gr[1], uc[1] * gr[0]), c.acc[4]);
-        c.acc[5] = fma(-tn_, fma(uc[0], gr[2], uc[2] * gr[0]), c.acc[5]);
-        c.acc[6] = fma(-tn_, 2.0 * uc[1] * gr[1], c.acc[6]);
-        c.acc[7] = fma(-tn_, fma(uc[1], gr[2], uc[2] * gr[1]), c.acc[7]);
-        c.acc[8] = fma(-tn_, 2.0 * uc[2] * gr[2], c.acc[8]);
-    }
-    // the neighbours' primitives of plane j are in registers: rows above and below may publish those of plane j+1
-    row_arrive_at<OY_OWN>(f.rowbar);
-  } else {
     // B: x and y faces of plane j (hi face per thread), both solvers in ONE basic block so that their
     // dependent chains interleave
     double Py[3] = {0.0, 0.0, 0.0}, EFy[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, usy[3] = {0.0, 0.0, 0.0};
@@ -1455,7 +1363,6 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         c.acc[8] = fma(-tn, 2.0 * uc[2] * gr[2], c.acc[8]);
     }
 
-  }
 
     // E: plane j+1 has arrived in ring slot `it`; z face (j, j+1); U*(j) complete -> the same slot;
     // publish primitives(j+1)
@@ -1483,7 +1390,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         Pi_n[0] = fma(-Un[1], u_n[0], Un[4]); Pi_n[1] = fma(-Un[1], u_n[1], Un[5]); Pi_n[2] = fma(-Un[1], u_n[2], Un[6]);
         Pi_n[3] = fma(-Un[2], u_n[1], Un[7]); Pi_n[4] = fma(-Un[2], u_n[2], Un[8]); Pi_n[5] = fma(-Un[3], u_n[2], Un[9]);
     }
-    if (EARLYPUB && !YRECOMP) {
+    if (EARLYPUB) {
         sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
         sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];
         row_arrive_at<OP_OWN>(f.rowbar);                              // primitives of plane j+1 of this row are published
@@ -1538,11 +1445,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
             c.wx0 = o[1]; c.wy0 = o[2];
         }
     }
-    if (YRECOMP) {       // the rows below and above have read the primitives of plane j
-        if (f.ty > 0) mbar_wait_at<OY_LO>(f.rowbar, it & 1);
-        if (f.ty < FY - 1) mbar_wait_at<OY_UP>(f.rowbar, it & 1);
-    }
-    if (!(EARLYPUB && !YRECOMP)) {
+    if (!EARLYPUB) {
         sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
         sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];
     }
@@ -1560,7 +1463,7 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
         for (int q = 0; q < 6; ++q) c.accP[q] = Pi_n[q];
         pi_source<2>(c.accP, Pi_n, usz, th2);
     }
-    if (!(EARLYPUB && !YRECOMP)) row_arrive_at<OP_OWN>(f.rowbar);     // primitives of plane j+1 of this row are published
+    if (!EARLYPUB) row_arrive_at<OP_OWN>(f.rowbar);     // primitives of plane j+1 of this row are published
 
     if (b.block_fix) {
         group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
@@ -1580,192 +1483,6 @@ __device__ __forceinline__ void bme_iter(const FusedArgs<NFB>& a, BlockTab* T, c
     if (f.tx == 0) mbar_arrive_at<8 * NS>(slotbar);   // this row's U*(j) is complete
 }
 
-#if GP_EROWS == 2
-// gravity source of the collisionless fields of one cell (reading G5): -tau n g_i and
-// -tau n [(u_i - tau g_i/2) g_j + (u_j - tau g_j/2) g_i]
-__device__ __forceinline__ void bme_gravity(BmeCarry& c, const double gr[3], double tau) {
-    double uc[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) uc[d] = fma(-0.5 * tau, gr[d], c.u[d]);
-    const double tn = tau * c.n;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) c.acc[d] = fma(-tn, gr[d], c.acc[d]);
-    c.acc[3] = fma(-tn, 2.0 * uc[0] * gr[0], c.acc[3]);
-    c.acc[4] = fma(-tn, fma(uc[0], gr[1], uc[1] * gr[0]), c.acc[4]);
-    c.acc[5] = fma(-tn, fma(uc[0], gr[2], uc[2] * gr[0]), c.acc[5]);
-    c.acc[6] = fma(-tn, 2.0 * uc[1] * gr[1], c.acc[6]);
-    c.acc[7] = fma(-tn, fma(uc[1], gr[2], uc[2] * gr[1]), c.acc[7]);
-    c.acc[8] = fma(-tn, 2.0 * uc[2] * gr[2], c.acc[8]);
-}
-
-// x face (hi; lo from the left lane) of one row and its flux differences
-__device__ __forceinline__ void bme_xface(BmeCarry& c, const BmeShared& S, int te, double th2, double th4) {
-    const double2 x0 = lds2(S.nu + 2 * te), x1 = lds2(S.uu + 2 * te), x2 = lds2(S.px + 2 * te);
-    const double urx[3] = {x0.y, x1.x, x1.y};
-    const double Plx[3] = {c.Pi[0], c.Pi[1], c.Pi[2]}, Prx[3] = {x2.x, S.pxy[te], x2.y};
-    double Px[3], EFx[6], usx[3];
-    bme_face<0>(c.n, c.u, Plx, x0.x, urx, Prx, Px, EFx, usx);
-#pragma unroll
-    for (int q = 0; q < 3; ++q) c.acc[q] -= th2 * (Px[q] - __shfl_up_sync(0xffffffffu, Px[q], 1));
-#pragma unroll
-    for (int q = 0; q < 6; ++q) c.acc[3 + q] -= th4 * (EFx[q] - __shfl_up_sync(0xffffffffu, EFx[q], 1));
-}
-
-// Two footprint rows per thread (rows 2w and 2w+1 of Eulerian warp w): the y face between them is solved once and
-// stays in registers, the face above the upper row goes to the warp above through shared memory as before.  Plain
-// scheme only (no GP_OVERDET).
-template <bool ST>
-__device__ __forceinline__ void bme_iter2(const FusedArgs<NFB>& a, BlockTab* T, const Blk& b, const Foot (&f)[2], const BmeShared& S,
-                                          BmeCarry (&c)[2], int j, double tau, double th, double inv2h) {
-    static_assert(!OD, "two rows per thread: plain scheme only");
-    const Geo& g = a.g;
-    const int w = threadIdx.x >> 5;
-    const int t0 = f[0].t, t1 = f[1].t, tx = f[0].tx;
-    const double th2 = 0.5 * th, th4 = 0.25 * th;
-    const bool zout = g.bcz == GP_BC_OUTFLOW;
-    const bool top_copy = !ST && zout && j == g.nz;
-    const bool bot_dup = !ST && zout && j == 0;
-    const bool do_out = ST || j - 1 >= b.z0;
-    const int it = j - (b.z0 - 1);
-    const double* ph0 = S.phi + pslot(it + 1) * PL;
-    const unsigned rowbar = f[0].rowbar;
-    if (it > 0 && w < NEW - 1) mbar_wait_at<OP_UP>(rowbar, (it - 1) & 1);   // primitives of plane j of the warp above are published
-
-    // B: the y face between the two rows (registers only), the y face above the upper row, the x faces of both rows
-    const bool s0 = f[0].star_row, s1 = f[1].star_row;      // warp 0: row 0 is halo; last warp: row 1 is halo
-    const int e0 = tx < FX - 1 ? t0 + 1 : t0, e1 = e0 + FX, w0 = tx > 0 ? t0 - 1 : t0, w1 = w0 + FX;
-    double Pym[3], EFym[6], usm[3];
-    {
-        const double Pl[3] = {c[0].Pi[1], c[0].Pi[3], c[0].Pi[4]}, Pr[3] = {c[1].Pi[1], c[1].Pi[3], c[1].Pi[4]};
-        bme_face<1>(c[0].n, c[0].u, Pl, c[1].n, c[1].u, Pr, Pym, EFym, usm);
-    }
-    double Pyh[3] = {0.0, 0.0, 0.0}, EFyh[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, ush[3];
-    if (s1) {
-        const int tn = t1 + FX;
-        const double2 y0 = lds2(S.nu + 2 * tn), y1 = lds2(S.uu + 2 * tn), y2 = lds2(S.py + 2 * tn);
-        const double ury[3] = {y0.y, y1.x, y1.y};
-        const double Pl[3] = {c[1].Pi[1], c[1].Pi[3], c[1].Pi[4]}, Pr[3] = {S.pxy[tn], y2.x, y2.y};
-        bme_face<1>(c[1].n, c[1].u, Pl, y0.x, ury, Pr, Pyh, EFyh, ush);
-        fy_store(S.fy, t1, Pyh, EFyh, ush);
-        bme_xface(c[1], S, e1, th2, th4);
-    }
-    if (s0) bme_xface(c[0], S, e0, th2, th4);
-    row_arrive_at<OY_OWN>(rowbar);                                    // y fluxes above this warp's upper row are written
-    if (w > 0) mbar_wait_at<OY_LO>(rowbar, it & 1);                 // ... and those above the warp below
-
-    // C: y-flux differences and the gravity source
-    if (s1) {
-#pragma unroll
-        for (int q = 0; q < 3; ++q) c[1].acc[q] -= th2 * (Pyh[q] - Pym[q]);
-#pragma unroll
-        for (int q = 0; q < 6; ++q) c[1].acc[3 + q] -= th4 * (EFyh[q] - EFym[q]);
-        const double gr[3] = {(ph0[e1] - ph0[w1]) * inv2h, (ph0[t1 + FX] - ph0[t0]) * inv2h,
-                              (S.phi[pslot(it + 2) * PL + t1] - S.phi[pslot(it) * PL + t1]) * inv2h};
-        bme_gravity(c[1], gr, tau);
-    }
-    if (s0) {
-        const double* fy = S.fy + 2 * (t0 - FX);
-        const double2 l0 = lds2(fy), l1 = lds2(fy + PP), l2 = lds2(fy + 2 * PP), l3 = lds2(fy + 3 * PP);
-        const double l4 = S.fy[4 * PP + t0 - FX];
-        c[0].acc[0] -= th2 * (Pym[0] - l0.x); c[0].acc[1] -= th2 * (Pym[1] - l0.y); c[0].acc[2] -= th2 * (Pym[2] - l1.x);
-        c[0].acc[3] -= th4 * (EFym[0] - l1.y); c[0].acc[4] -= th4 * (EFym[1] - l2.x); c[0].acc[5] -= th4 * (EFym[2] - l2.y);
-        c[0].acc[6] -= th4 * (EFym[3] - l3.x); c[0].acc[7] -= th4 * (EFym[4] - l3.y); c[0].acc[8] -= th4 * (EFym[5] - l4);
-        const double gr[3] = {(ph0[e0] - ph0[w0]) * inv2h, (ph0[t1] - ph0[t0 - FX]) * inv2h,
-                              (S.phi[pslot(it + 2) * PL + t0] - S.phi[pslot(it) * PL + t0]) * inv2h};
-        bme_gravity(c[0], gr, tau);
-    }
-
-    // E: plane j+1 has arrived in ring slot `it`; row by row: primitives of plane j+1, z face (j, j+1), U*(j) complete
-    double* rs = S.ring + rslot(it) * BmeTraits::SLOT;
-    const unsigned slotbar = f[0].tabbar + 8 * rslot(it);
-    mbar_wait_at<0>(slotbar, rpar(it));
-#pragma unroll
-    for (int q = 0; q < 2; ++q) {
-        const int t = f[q].t;
-        BmeCarry& cq = c[q];
-        double Un[NBME];
-#pragma unroll
-        for (int P = 0; P < 5; ++P) {
-            const double2 sp = lds2(rs + P * PP + 2 * t);
-            Un[2 * P] = sp.x; Un[2 * P + 1] = sp.y;
-        }
-        const double n_n = Un[0], in_n = frcp(n_n);
-        const double u_n[3] = {Un[1] * in_n, Un[2] * in_n, Un[3] * in_n};
-        double Pi_n[6];
-        Pi_n[0] = fma(-Un[1], u_n[0], Un[4]); Pi_n[1] = fma(-Un[1], u_n[1], Un[5]); Pi_n[2] = fma(-Un[1], u_n[2], Un[6]);
-        Pi_n[3] = fma(-Un[2], u_n[1], Un[7]); Pi_n[4] = fma(-Un[2], u_n[2], Un[8]); Pi_n[5] = fma(-Un[3], u_n[2], Un[9]);
-        sts2(S.nu + 2 * t, n_n, u_n[0]); sts2(S.uu + 2 * t, u_n[1], u_n[2]); sts2(S.px + 2 * t, Pi_n[0], Pi_n[2]);
-        sts2(S.py + 2 * t, Pi_n[3], Pi_n[4]); S.pxy[t] = Pi_n[1];
-        double Pz[3] = {0.0, 0.0, 0.0}, EFz[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, usz[3];
-        if (f[q].star_row) {
-            const double Pl[3] = {cq.Pi[2], cq.Pi[4], cq.Pi[5]};
-            const double Pr[3] = {Pi_n[2], Pi_n[4], Pi_n[5]};
-            bme_face<2>(cq.n, cq.u, Pl, n_n, u_n, Pr, Pz, EFz, usz);
-            double o[NBME];      // n, w (3), nE (6)
-            if (top_copy) {                       // outflow: U*(nz) := U*(nz-1)
-                const double* rq = S.ring + rslot(it + NS - 1) * BmeTraits::SLOT;
-                const double2 q0 = lds2(rq + 2 * t), q1 = lds2(rq + PP + 2 * t);
-                o[0] = q0.x; o[3] = q0.y; o[1] = q1.x; o[2] = q1.y;
-#pragma unroll
-                for (int P = 2; P < 5; ++P) {
-                    const double2 qp = lds2(rq + P * PP + 2 * t);
-                    o[2 * P] = qp.x; o[2 * P + 1] = qp.y;
-                }
-            } else {
-                o[0] = cq.n;
-#pragma unroll
-                for (int d = 0; d < 3; ++d) o[1 + d] = fma(-th2, Pz[d], cq.acc[d]) * cq.in;
-#pragma unroll
-                for (int k = 0; k < 6; ++k) o[4 + k] = fma(-th4, EFz[k], cq.acc[3 + k]);
-            }
-            sts2(rs + 2 * t, o[0], o[3]); sts2(rs + PP + 2 * t, o[1], o[2]);
-#pragma unroll
-            for (int P = 2; P < 5; ++P) sts2(rs + P * PP + 2 * t, o[2 * P], o[2 * P + 1]);
-            if (bot_dup) {                        // outflow: U*(-1) := U*(0)
-                double* rg = S.ring + rslot(it + NS - 1) * BmeTraits::SLOT;
-                sts2(rg + 2 * t, o[0], o[3]); sts2(rg + PP + 2 * t, o[1], o[2]);
-#pragma unroll
-                for (int P = 2; P < 5; ++P) sts2(rg + P * PP + 2 * t, o[2 * P], o[2 * P + 1]);
-            }
-            if (do_out) {                         // 4 x z-average of w*_x, w*_y for plane j-1
-                const double2 wm = lds2(S.ring + rslot(it + NS - 2) * BmeTraits::SLOT + PP + 2 * t);
-                const double2 wc = lds2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + PP + 2 * t);
-                sts2(S.tz + (it % NTZ) * PP + 2 * t, sum3(wm.x, wc.x, o[1]), sum3(wm.y, wc.y, o[2]));
-            }
-        }
-#pragma unroll
-        for (int d = 0; d < 3; ++d) cq.acc[d] = fma(th2, Pz[d], Un[1 + d]);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) cq.acc[3 + k] = fma(th4, EFz[k], Un[4 + k]);
-        cq.n = n_n; cq.in = in_n;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) cq.u[d] = u_n[d];
-#pragma unroll
-        for (int k = 0; k < 6; ++k) cq.Pi[k] = Pi_n[k];
-    }
-    row_arrive_at<OP_OWN>(rowbar);                                    // primitives of plane j+1 of both rows are published
-
-    if (b.block_fix) {
-        group_sync(&T->esync, 1);                  // phases: prologue 0, then two per plane
-#pragma unroll
-        for (int q = 0; q < 2; ++q)
-            if (f[q].fix) {
-                const int t = f[q].t, src = f[q].fix_src;
-#pragma unroll
-                for (int P = 0; P < 5; ++P) {
-                    const double2 v = lds2(rs + P * PP + 2 * src);
-                    sts2(rs + P * PP + 2 * t, v.x, v.y);
-                    if (bot_dup) sts2(S.ring + rslot(it + NS - 1) * BmeTraits::SLOT + P * PP + 2 * t, v.x, v.y);
-                }
-                const double2 v = lds2(S.tz + (it % NTZ) * PP + 2 * src);
-                sts2(S.tz + (it % NTZ) * PP + 2 * t, v.x, v.y);
-            }
-        group_sync(&T->esync, 0);
-    }
-    __syncwarp();
-    if (tx == 0) mbar_arrive_at<8 * NS>(slotbar);   // this warp's U*(j) is complete
-}
-#endif  // GP_EROWS == 2
 
 __global__ void __launch_bounds__(NT, 1)
 k_fused_bme(const __grid_constant__ FusedArgs<NFB> a) {
@@ -1806,27 +1523,15 @@ k_fused_bme(const __grid_constant__ FusedArgs<NFB> a) {
         reg_alloc<GP_REG_E>();
 #endif
         if ((int)threadIdx.x < NEW * 32) {
-#if GP_EROWS == 2
-        const int w = threadIdx.x >> 5;
-        const Foot f[2] = {make_foot(g, b, T, 2 * w), make_foot(g, b, T, 2 * w + 1)};
-        BmeCarry c[2] = {bme_prologue(a, g, b, f[0], S, th), bme_prologue(a, g, b, f[1], S, th)};
-#else
         const Foot f = make_foot(g, b, T, threadIdx.x >> 5);
         BmeCarry c = bme_prologue(a, g, b, f, S, th);
-#endif
         mbar_wait(&T->pro, 0);
         group_sync(&T->esync, 0);
 
         int j = b.z0 - 1;
-#if GP_EROWS == 2
-        for (; j <= b.z0 && j <= b.z1; ++j) bme_iter2<false>(a, T, b, f, S, c, j, tau, th, inv2h);
-        for (; j <= b.z1 - 1; ++j) bme_iter2<true>(a, T, b, f, S, c, j, tau, th, inv2h);
-        for (; j <= b.z1; ++j) bme_iter2<false>(a, T, b, f, S, c, j, tau, th, inv2h);
-#else
         for (; j <= b.z0 && j <= b.z1; ++j) bme_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1 - 1; ++j) bme_iter<true>(a, T, b, f, S, c, j, tau, th, inv2h);
         for (; j <= b.z1; ++j) bme_iter<false>(a, T, b, f, S, c, j, tau, th, inv2h);
-#endif
         }   // real Eulerian warps (the padding warps of the register split skip to the reduction)
     }
     block_max_commit(smax, bad, a.smax_bits, a.flag, S.nu, kap, a.kappa);
