@@ -301,6 +301,9 @@ void lagrangian(orc_ctx* c, double tau) {
 // ---------------------------------------------------------------------------------------------
 // S4 CFL (reading G4; wave speeds PAPER.md:86 and 140):
 //   dt = cfl * h / max_{cells, d} ( |v_d| + sqrt(gamma p / rho),  |u_d| + sqrt(3 Pi_dd / n) )
+// With the overdetermined system enabled (reading G16) p and Pi_dd are the ones the stages use, i.e. those of the
+// carried fields: p = (gamma-1) rho*eps (PAPER.md:41 last line), Pi_dd carried by PAPER.md:65; the state is
+// reported unphysical when THEY are not positive, not when the total-energy description is not.
 // ---------------------------------------------------------------------------------------------
 int max_dt(orc_ctx* c, double cfl, double* dt) {
     double smax = 0.0;
@@ -310,7 +313,8 @@ int max_dt(orc_ctx* c, double cfl, double* dt) {
             for (int i = 0; i < c->nx; ++i) {
                 const std::size_t q = c->at(i, j, k);
                 if (c->has_gas()) {
-                    const GasPrim w = gas_prim(c, c->U, q);
+                    GasPrim w = gas_prim(c, c->U, q);
+                    if (c->od) w.p = (c->gamma - 1.0) * c->eps[q];      // G16: the pressure the stages use
                     if (!(w.rho > 0.0) || !(w.p > 0.0) || !std::isfinite(w.rho) || !std::isfinite(w.p)) bad = true;
                     const double cs = std::sqrt(c->gamma * w.p / w.rho);
                     for (int d = 0; d < 3; ++d) {
@@ -323,7 +327,7 @@ int max_dt(orc_ctx* c, double cfl, double* dt) {
                     const BmePrim w = bme_prim(c->U, q);
                     if (!(w.n > 0.0) || !std::isfinite(w.n)) bad = true;
                     for (int d = 0; d < 3; ++d) {
-                        const double Pdd = w.Pi[sym(d, d)];
+                        const double Pdd = c->od ? c->Pi[sym(d, d)][q] : w.Pi[sym(d, d)];   // G16
                         if (!(Pdd > 0.0)) bad = true;
                         const double s = std::fabs(w.u[d]) + std::sqrt(3.0 * Pdd / w.n);
                         if (!std::isfinite(s)) bad = true;

@@ -244,6 +244,51 @@ def test_balance_of_the_collisionless_component_by_hand(orc):
     assert o.kappa()[1] <= 1e-14
 
 
+def test_cfl_of_an_overdetermined_context_uses_the_carried_fields(orc):
+    """Reading G16: with the overdetermined system on, the signal speeds are those of the pressure and dispersion the
+    stages use, p = (gamma-1) rho*eps and the carried Pi_dd.  A state whose total-energy description is unphysical in
+    a block (gas-vacuum border) but whose carried fields are positive yields a finite dt, equal to the brute-force
+    maximum over the carried-field wave speeds; a non-positive CARRIED value is what gets reported."""
+    g = 1.4
+    w = W.smooth_gas(dims=(12, 8, 6), kmax=2, amp=0.3, components=W.GAS | W.STARS, gamma=g)
+    st = w.state()
+    base = make(orc, w)
+    o = make(orc, w)
+    o.od_enable()
+    dt0 = base.max_dt(0.3)
+    assert o.max_dt(0.3) == pytest.approx(dt0, rel=1e-14)        # derived carried fields: the same speeds
+    rng = np.random.default_rng(11)
+    eps = o.get("eps") * rng.uniform(0.5, 2.0, size=st["rho"].shape)
+    P = {k: o.get(k) * rng.uniform(0.5, 2.0, size=st["rho"].shape) for k in ("Pxx", "Pyy", "Pzz")}
+    E = st["E"].copy()
+    E[1:3, 2:5, 3:9] = 1e-3                                     # far below the kinetic energy there
+    Exx = st["Exx"].copy()
+    Exx[3:5, 2:5, 3:9] = 1e-3
+    o.set("eps", eps); o.set("E", E); o.set("Exx", Exx)
+    for k, a in P.items():
+        o.set(k, a)
+    base.set("E", E)
+    with pytest.raises(Exception):
+        base.max_dt(0.3)                                        # the base scheme rightly reports the state
+    v = [np.abs(st[k] / st["rho"]) for k in ("mx", "my", "mz")]
+    u = [np.abs(st[k] / st["n"]) for k in ("nux", "nuy", "nuz")]
+    cs = np.sqrt(g * (g - 1.0) * eps / st["rho"])
+    smax = max(max((a + cs).max() for a in v),
+               max((a + np.sqrt(3.0 * P[k] / st["n"])).max() for a, k in zip(u, ("Pxx", "Pyy", "Pzz"))))
+    assert o.max_dt(0.3) == pytest.approx(0.3 * w.h / smax, rel=1e-14)
+    assert abs(o.max_dt(0.3) - dt0) > 1e-3 * dt0                # and it is not the base scheme's number
+    for name in ("eps", "Pyy"):
+        a = o.get(name)
+        keep = a[2, 3, 4]
+        a[2, 3, 4] = -keep
+        o.set(name, a)
+        with pytest.raises(Exception):
+            o.max_dt(0.3)
+        a[2, 3, 4] = keep
+        o.set(name, a)
+    assert np.isfinite(o.max_dt(0.3))
+
+
 def test_dispersion_equation_agrees_with_the_energy_tensor_on_smooth_shear(orc):
     """One unbalanced step of a smooth state with all six Pi components and all velocities varying: the Pi_ij carried by
     PAPER.md:65 and the one implied by n E_ij differ by the truncation error only, first order in h."""
