@@ -91,7 +91,9 @@ int gp_solve_poisson(gp_ctx* ctx);
  * (|u_d| + sqrt(3 Pi_dd/n)) (wave speeds PAPER.md:86, 140).  The result stays on the device
  * for gp_step(ctx, 0).  If `dt` is not NULL the call also copies it to *dt (host pointer),
  * synchronises, and returns GP_ERR_STATE if the state holds NaN/Inf or a non-positive
- * rho, n, p or Pi_dd. */
+ * rho, n, p or Pi_dd.  In a GP_OD context p and Pi_dd are those of the CARRIED fields, the ones the stages
+ * use: p = (gamma-1) rho*eps and the carried Pi_dd (reading G16); a cell whose total-energy description
+ * is unphysical but whose carried fields are positive (gas-vacuum border) is then not an error. */
 int gp_max_dt(gp_ctx* ctx, double cfl, double* dt);
 
 /* One timestep: Eulerian stage (face values PAPER.md:112-114 and
@@ -124,7 +126,13 @@ int gp_step(gp_ctx* ctx, double dt);
  *   synchronises).  A component that is not enabled reports 0.
  * gp_od_last_kappa: the same two sums for the state the last gp_od_step / gp_step produced BEFORE its balance was
  *   applied, folded by the step kernels at no extra pass (the paper's per-step check); GP_ERR_STATE if no step has
- *   run since the state was last set. */
+ *   run since the state was last set.  The blocks of the step kernels add their partial sums with one fp64
+ *   atomicAdd each, in scheduling order: unlike gp_kappa (fixed-order sum, bit-reproducible) the last digits of
+ *   these two numbers may differ from run to run (relative 1e-15 or so); the state itself is deterministic.
+ * Stale carried fields: writing a conserved field of a GP_OD context with gp_set_state leaves the carried fields of
+ *   that component behind (and fresh storage holds none at all).  Until gp_od_derive has run, or the carried fields
+ *   have been set as well, gp_step / gp_od_step, gp_max_dt and gp_od_balance return GP_ERR_STATE instead of
+ *   computing with the pressure of some other state. */
 int gp_od_derive(gp_ctx* ctx);
 int gp_od_step(gp_ctx* ctx, double dt, int balance);
 int gp_od_balance(gp_ctx* ctx);

@@ -73,6 +73,25 @@ static bool field_enabled(const gp_grid& g, int f) {
     return f < NGAS ? (g.components & GP_GAS) != 0 : (g.components & GP_STARS) != 0;
 }
 
+// Carried fields of a GP_OD context that do not follow the conserved ones (bit f - F_EPS per internal field f).
+// A carried field goes stale when a conserved field of its component is written through gp_set_state, and is fresh
+// again once gp_od_derive has run or the field itself has been set.  While any bit is set, gp_step / gp_od_step,
+// gp_max_dt and gp_od_balance refuse (GP_ERR_STATE): a step would otherwise run on the pressure of another state
+// (or on p = 0 of fresh storage) and the balance would then overwrite the evidence.
+static unsigned od_all_stale(const gp_grid& g) {
+    if (!(g.components & GP_OD)) return 0u;
+    unsigned m = 0u;
+    if (g.components & GP_GAS) m |= 1u;                      // rho*eps
+    if (g.components & GP_STARS) m |= 0x3fu << 1;            // Pi_xx ... Pi_zz
+    return m;
+}
+static int od_check_fresh(const gp_ctx* c, const char* who) {
+    if (!c->od_stale) return GP_OK;
+    set_error("%s: the carried fields (rho*eps / Pi_ij) of this GP_OD context do not follow the conserved fields that were "
+              "set since (stale mask 0x%x): call gp_od_derive, or set them with gp_set_state(GP_EPS ... GP_PZZ)", who, c->od_stale);
+    return GP_ERR_STATE;
+}
+
 static size_t storage_bytes(const gp_grid& g) {
     const size_t N = (size_t)g.nx * g.ny * g.nz;
     const size_t fb = align256(N * sizeof(double));
@@ -144,6 +163,7 @@ static int ensure_storage(gp_ctx* c) {
     c->phip = (double*)take(phi_pad_elems(g.nx, g.ny, g.nz) * sizeof(double)) + (PHI_XOFF - 2);   // interior rows 128-byte aligned
     c->d_kappa = (double*)take(256);
     c->kappa_cached = false;
+    c->od_stale = od_all_stale(c->g);
     char* small = take(256);
     c->d_dt = (double*)small;
     c->d_smax = (unsigned long long*)(small + 64);
@@ -255,6 +275,7 @@ void gp_destroy(gp_ctx* c) {
     if (c->ready || c->fft_ready) cudaStreamSynchronize(c->stream);
     poisson_teardown(c);
     if (c->owns && c->base) cudaFree(c->base);
+    delete c->tmc[0]; delete c->tmc[1];
     if (c->tim) {
         for (size_t i = 0; i < 2 * c->tim->cap; ++i) cudaEventDestroy(c->tim->ev[i]);
         delete[] c->tim->ev; delete[] c->tim->kid;
@@ -361,6 +382,10 @@ int gp_set_state(gp_ctx* c, int field, const double* src, int on_device) {
     c->cfl_cached = false;
     c->src_cached = false;
     c->kappa_cached = false;
+    if (c->od) {
+        if (fi >= F_EPS) c->od_stale &= ~(1u << (fi - F_EPS));                  // this carried field is the caller's now
+        else c->od_stale |= od_all_stale(c->g) & (fi < NGAS ? 1u : 0x3fu << 1); // its component's carried fields lag
+    }
     return GP_OK;
 }
 
@@ -398,6 +423,7 @@ int gp_max_dt(gp_ctx* c, double cfl, double* dt) {
     if (!c || !(cfl > 0.0)) { set_error("gp_max_dt: bad argument"); return GP_ERR_ARG; }
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
+    if (c->od && (rc = od_check_fresh(c, "gp_max_dt")) != GP_OK) return rc;    // reads the carried fields (G16)
     // after a step the fused kernels have already folded the max signal speed of the new state
     rc = c->cfl_cached ? launch_cfl_from_cache(c, cfl) : launch_cfl(c, cfl);
     if (rc != GP_OK) return rc;
@@ -418,6 +444,7 @@ static int step_impl(gp_ctx* c, double dt, int od_balance) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     const bool od = od_balance >= 0;
+    if (od && (rc = od_check_fresh(c, "gp_step")) != GP_OK) return rc;
     const double* d_dt = dt > 0.0 ? nullptr : c->d_dt;
     if ((rc = launch_cfl_reset_next(c)) != GP_OK) return rc;
     if (od) GP_CUDA(cudaMemsetAsync(c->d_kappa, 0, 2 * sizeof(double), c->stream));
@@ -467,6 +494,7 @@ int gp_od_derive(gp_ctx* c) {
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
     c->kappa_cached = false;
+    c->od_stale = 0u;
     return launch_od_derive(c);
 }
 
@@ -474,6 +502,7 @@ int gp_od_balance(gp_ctx* c) {
     GP_NEED_OD("gp_od_balance");
     int rc = ensure_storage(c);
     if (rc != GP_OK) return rc;
+    if ((rc = od_check_fresh(c, "gp_od_balance")) != GP_OK) return rc;
     c->cfl_cached = false;       // the balance may change momenta and energies
     c->kappa_cached = false;
     return launch_od_balance(c);

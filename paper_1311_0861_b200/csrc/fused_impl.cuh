@@ -44,6 +44,9 @@
 #include <cuda.h>
 
 #include <cstddef>
+#include <cstring>
+#include <mutex>
+#include <new>
 
 #include "gp_internal.h"
 
@@ -714,7 +717,7 @@ struct GasTraits {
         if (LAST1) a.Un[4][off] = out[4];
         if (a.src_out) a.src_out[off] = out[0] + n_other;
         // CFL of the new state (reading G4)
-        const double pn = gm1 * (out[4] - kin);
+        const double pn = OD ? gm1 * out[IEPS] : gm1 * (out[4] - kin);   // GP_OD: the carried pressure (reading G16)
         const double c2 = a.gamma * pn * irn;
         const double sp = fmax(fmax(fabs(ux), fabs(uy)), fabs(uz)) + c2 * frsqrt(c2);
         if (!(out[0] > 0.0) || !(pn > 0.0) || !(sp <= 1.7976931348623157e308)) bad = 1;
@@ -1189,7 +1192,7 @@ struct BmeTraits {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             const double ud = out[1 + d] * inn;
-            const double Pdd = fma(-out[1 + d], ud, out[dd[d]]);
+            const double Pdd = OD ? out[PI0 + dd[d] - 4] : fma(-out[1 + d], ud, out[dd[d]]);   // GP_OD: carried (G16)
             const double c2 = 3.0 * Pdd * inn;
             const double sp = fabs(ud) + c2 * frsqrt(c2);
             if (!(Pdd > 0.0) || !(sp <= 1.7976931348623157e308)) bad = 1;
@@ -1559,7 +1562,8 @@ static int pick_zchunk(const gp_ctx* c, int tiles_xy) {
     return best;
 }
 
-// Tensor maps of one launch (host side, a few microseconds): field pairs as rows of 2 nx doubles, the gas energy and
+// Tensor maps of one launch (host side; encoded at the first launch on each half of the double buffer, then taken
+// from the context's TmCache): field pairs as rows of 2 nx doubles, the gas energy and
 // the padded Phi as rows of doubles; boxes of one footprint plane.  Returns false if TMA cannot describe the grid
 // (odd nx: rows not 16-byte aligned) or the driver entry point is missing; the kernel then stages cell by cell.
 typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -1568,14 +1572,13 @@ typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, v
 
 static bool encode_map(CUtensorMap* tm, const void* base, size_t row_doubles, size_t ny, size_t nz, unsigned box_doubles) {
     static EncodeTiled enc = nullptr;
-    static bool looked = false;
-    if (!looked) {
+    static std::once_flag looked;
+    std::call_once(looked, [] {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
             enc = (EncodeTiled)fn;
-        looked = true;
-    }
+    });
     if (!enc || (row_doubles & 1)) return false;
     const cuuint64_t dims[3] = {row_doubles, ny, nz};
     const cuuint64_t strides[2] = {row_doubles * sizeof(double), row_doubles * ny * sizeof(double)};
@@ -1585,7 +1588,7 @@ static bool encode_map(CUtensorMap* tm, const void* base, size_t row_doubles, si
 }
 
 template <int NF, class K>
-static int launch_fused_t(gp_ctx* c, K kernel, const int* fields, int planes, int kid, double dt, const double* d_dt,
+static int launch_fused_t(gp_ctx* c, int which, K kernel, const int* fields, int planes, int kid, double dt, const double* d_dt,
                           const double* src_in = nullptr, double* src_out = nullptr, int balance = 0, double* kappa = nullptr) {
     FusedArgs<NF> a;
     a.src_in = src_in; a.src_out = src_out;
@@ -1593,11 +1596,32 @@ static int launch_fused_t(gp_ctx* c, K kernel, const int* fields, int planes, in
     a.g = Geo{c->g.nx, c->g.ny, c->g.nz, c->bc.x, c->bc.y, c->bc.z};
     for (int f = 0; f < NF; ++f) { a.U[f] = c->U[fields[f]]; a.Un[f] = c->Us[fields[f]]; }
     a.phi = phipad_of(c);
-    bool ok = true;
-    for (int P = 0; P < NF / 2; ++P) ok = ok && encode_map(&a.tm[P], a.U[2 * P], 2 * (size_t)c->g.nx, c->g.ny, c->g.nz, 2 * FX);
-    if (NF & 1) ok = ok && encode_map(&a.tm[NF / 2], a.U[NF - 1], c->g.nx, c->g.ny, c->g.nz, FX);
-    ok = ok && encode_map(&a.tm[(NF + 1) / 2], a.phi.p, a.phi.pitch, a.phi.py, (size_t)c->g.nz + 4, FX);
-    a.use_tma = ok ? 1 : 0;
+    // tensor maps: encoded once per half of the double buffer and kept with the context (gp_internal.h, TmCache)
+    constexpr int NTM = (NF + 1) / 2 + 1;
+    static_assert(NTM <= TM_MAX, "TmCache holds every map of one launch");
+    TmCache*& tc = c->tmc[which];
+    if (!tc) { tc = new (std::nothrow) TmCache; if (tc) std::memset((void*)tc, 0, sizeof(*tc)); }
+    int set = -1;
+    if (tc)
+        for (int q = 0; q < 2; ++q)
+            if (tc->key_u[q] == (const void*)a.U[0] && tc->key_phi[q] == (const void*)a.phi.p) set = q;
+    if (set < 0) {
+        CUtensorMap* tm = tc ? tc->tm[tc->next] : a.tm;
+        bool ok = true;
+        for (int P = 0; P < NF / 2; ++P) ok = ok && encode_map(&tm[P], a.U[2 * P], 2 * (size_t)c->g.nx, c->g.ny, c->g.nz, 2 * FX);
+        if (NF & 1) ok = ok && encode_map(&tm[NF / 2], a.U[NF - 1], c->g.nx, c->g.ny, c->g.nz, FX);
+        ok = ok && encode_map(&tm[(NF + 1) / 2], a.phi.p, a.phi.pitch, a.phi.py, (size_t)c->g.nz + 4, FX);
+        a.use_tma = ok ? 1 : 0;
+        if (tc) {
+            set = tc->next;
+            tc->key_u[set] = a.U[0]; tc->key_phi[set] = a.phi.p; tc->ok[set] = a.use_tma;
+            tc->next ^= 1;
+        }
+    }
+    if (tc) {
+        a.use_tma = tc->ok[set];
+        std::memcpy((void*)a.tm, (const void*)tc->tm[set], NTM * sizeof(CUtensorMap));
+    }
     a.h = c->g.h; a.gamma = c->gamma; a.dt_val = dt; a.dt_ptr = d_dt;
     a.smax_bits = c->d_smax_next; a.flag = c->d_flag_next;
     const int tx = (c->g.nx + TXO - 1) / TXO, ty = (c->g.ny + TYO - 1) / TYO;
@@ -1617,7 +1641,7 @@ static int launch_fused_t(gp_ctx* c, K kernel, const int* fields, int planes, in
 #ifdef GP_FUSED_GAS
 static int launch_gas_impl(gp_ctx* c, double dt, const double* d_dt, const double* src_in, double* src_out, int balance) {
     const int fields[NGAS + NODG] = {0, 1, 2, 3, 4, F_EPS};
-    return launch_fused_t<NFG>(c, k_fused_gas, fields, GasTraits::PLANES, K_FUSED_GAS, dt, d_dt, src_in, src_out, balance,
+    return launch_fused_t<NFG>(c, 0, k_fused_gas, fields, GasTraits::PLANES, K_FUSED_GAS, dt, d_dt, src_in, src_out, balance,
                                OD ? c->d_kappa : nullptr);
 }
 #endif
@@ -1626,7 +1650,7 @@ static int launch_bme_impl(gp_ctx* c, double dt, const double* d_dt, int balance
     int fields[NBME + NODB];
     for (int f = 0; f < NBME; ++f) fields[f] = NGAS + f;
     for (int q = 0; q < NODB; ++q) fields[NBME + q] = F_PI + q;
-    return launch_fused_t<NFB>(c, k_fused_bme, fields, BmeTraits::PLANES, K_FUSED_BME, dt, d_dt, nullptr, nullptr, balance,
+    return launch_fused_t<NFB>(c, 1, k_fused_bme, fields, BmeTraits::PLANES, K_FUSED_BME, dt, d_dt, nullptr, nullptr, balance,
                                OD ? c->d_kappa + 1 : nullptr);
 }
 #endif

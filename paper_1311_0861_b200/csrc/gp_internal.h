@@ -2,6 +2,7 @@
 // nothing here is seen by oracle/).
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cufft.h>
 
@@ -88,6 +89,19 @@ struct Timing {
 
 }  // namespace gp
 
+namespace gp {
+// Tensor maps of one fused kernel, kept per context: nothing in them changes from step to step except the base
+// addresses, which alternate between the two halves of the double buffer, so two sets cover every launch.
+constexpr int TM_MAX = 9;      // 8 pair maps of the 16-field collisionless kernel + Phi
+struct TmCache {
+    const void* key_u[2];      // U[first field] the set was encoded for (null: empty)
+    const void* key_phi[2];
+    int ok[2];                 // TMA can describe the grid (else the kernel stages cell by cell)
+    int next;                  // set to overwrite next
+    alignas(64) CUtensorMap tm[2][TM_MAX];
+};
+}  // namespace gp
+
 struct gp_ctx {
     gp_grid g;
     double gamma;
@@ -112,6 +126,8 @@ struct gp_ctx {
     int* d_flag_next;
     double* d_kappa;                // GP_OD: [0..1] kappa_gas, kappa_bme folded by the last step (before its balance), [2..3] of gp_kappa
     bool kappa_cached;
+    unsigned od_stale;              // GP_OD: bit (f - F_EPS) set = carried field f has not followed the conserved fields
+                                    // (fresh storage, or a conserved field written since); see api.cu
     bool cfl_cached;                // d_smax_next / d_flag_next describe the current state
 
     // Poisson
@@ -129,6 +145,7 @@ struct gp_ctx {
     double* src;                    // periodic, gas + stars: rho + n assembled here (by the fused step or k_source)
     bool src_cached;                // src holds rho + n of the current state (written by the fused step)
 
+    gp::TmCache* tmc[2];            // tensor-map sets of the gas / collisionless fused kernel (fused_impl.cuh)
     long long n_own, n_fft;
     gp::Timing* tim;
 };

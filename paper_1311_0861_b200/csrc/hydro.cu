@@ -30,18 +30,21 @@ __device__ __forceinline__ GasPrim gas_prim(const ConstFields<NGAS>& U, size_t c
 
 // --------------------------------------------------------------------------------------------
 // CFL reduction (reading G4): max over cells and axes of |v_d| + sqrt(gamma p/rho) and
-// |u_d| + sqrt(3 Pi_dd/n).  Speeds are non-negative, so their bit patterns order like the
-// values and one atomicMax on the 64-bit pattern finishes the reduction.
+// |u_d| + sqrt(3 Pi_dd/n); in a GP_OD context p and Pi_dd are the carried ones (reading G16).  Speeds are
+// non-negative, so their bit patterns order like the values and one atomicMax on the 64-bit pattern finishes
+// the reduction.
 // --------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_cfl(size_t N, int has_gas, int has_stars, ConstFields<NGAS> Ug, int estr, ConstFields<NBME> Ub, double gamma,
+      const double* __restrict__ eps, ConstFields<3> Pdd_carried,
       unsigned long long* __restrict__ smax_bits, int* __restrict__ flag) {
     double smax = 0.0;
     int bad = 0;
     const double gm1 = gamma - 1.0;
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (size_t)gridDim.x * blockDim.x) {
         if (has_gas) {
-            const GasPrim w = gas_prim(Ug, c, gm1, estr);
+            GasPrim w = gas_prim(Ug, c, gm1, estr);
+            if (eps) w.p = gm1 * eps[BSTR * c];        // GP_OD (reading G16): the pressure the stages use
             if (!(w.rho > 0.0) || !(w.p > 0.0)) bad = 1;
             const double cs = sqrt(gamma * w.p / w.rho);
 #pragma unroll
@@ -58,7 +61,8 @@ k_cfl(size_t N, int has_gas, int has_stars, ConstFields<NGAS> Ug, int estr, Cons
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const double u = Ub.p[1 + d][BSTR * c] * in;
-                const double Pdd = Ub.p[4 + sym(d, d)][BSTR * c] - nn * u * u;
+                const double Pdd = Pdd_carried.p[d] ? Pdd_carried.p[d][BSTR * c]      // GP_OD (reading G16)
+                                                    : Ub.p[4 + sym(d, d)][BSTR * c] - nn * u * u;
                 if (!(Pdd > 0.0)) bad = 1;
                 const double s = fabs(u) + sqrt(3.0 * Pdd * in);
                 if (!(s <= 1.7976931348623157e308)) bad = 1;
@@ -159,12 +163,17 @@ int launch_cfl(gp_ctx* c, double cfl) {
     ConstFields<NGAS> Ug; ConstFields<NBME> Ub;
     for (int f = 0; f < NGAS; ++f) Ug.p[f] = c->U[f];
     for (int f = 0; f < NBME; ++f) Ub.p[f] = c->U[NGAS + f];
+    // GP_OD: signal speeds and the bad-state flag from the carried rho*eps and Pi_xx, Pi_yy, Pi_zz
+    const double* eps = (c->od && (c->g.components & GP_GAS)) ? c->U[F_EPS] : nullptr;
+    ConstFields<3> Pc;
+    const int diag[3] = {0, 3, 5};
+    for (int d = 0; d < 3; ++d) Pc.p[d] = (c->od && (c->g.components & GP_STARS)) ? c->U[F_PI + diag[d]] : nullptr;
     tic(c, K_CFL);
     k_cfl_begin<<<1, 1, 0, c->stream>>>(c->d_smax, c->d_flag);
     size_t blocks = (c->N + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
     k_cfl<<<(unsigned)blocks, 256, 0, c->stream>>>(c->N, (c->g.components & GP_GAS) != 0, (c->g.components & GP_STARS) != 0,
-                                                   Ug, c->estr, Ub, c->gamma, c->d_smax, c->d_flag);
+                                                   Ug, c->estr, Ub, c->gamma, eps, Pc, c->d_smax, c->d_flag);
     k_cfl_finish<<<1, 1, 0, c->stream>>>(c->d_smax, c->d_flag, c->d_flag, cfl, c->g.h, c->d_dt);
     toc(c);
     c->n_own += 3;

@@ -142,6 +142,25 @@ int poisson_setup(gp_ctx* c) {
     const int pitch = phi_pitch(nx), py = ny + 4;      // the inverse transform writes into the padded Phi
     if (c->g.poisson == GP_POISSON_PERIODIC) {
         c->zfused = zpass_supported(nz);
+        // The table uploads come first: a failure here returns before any plan exists, so nothing is left
+        // behind for a retry to leak (the plans are created last and cleaned up by the rc path below).
+        const double pi = 3.14159265358979323846;
+        std::vector<double> t((size_t)nx + ny + nz);
+        for (int k = 0; k < nx; ++k) { const double s = std::sin(pi * k / nx); t[k] = 1.0 - 2.0 / 3.0 * s * s; }
+        for (int k = 0; k < ny; ++k) { const double s = std::sin(pi * k / ny); t[nx + k] = 1.0 - 2.0 / 3.0 * s * s; }
+        for (int k = 0; k < nz; ++k) { const double s = std::sin(pi * k / nz); t[nx + ny + k] = 1.0 - 2.0 / 3.0 * s * s; }
+        GP_CUDA(cudaMemcpyAsync(c->tabx, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        GP_CUDA(cudaStreamSynchronize(c->stream));
+        if (c->zfused) {
+            std::vector<double> w(2 * (size_t)nz);
+            for (int k = 0; k < nz; ++k) {
+                const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)nz;
+                w[2 * k] = (double)cosl(a);
+                w[2 * k + 1] = (double)-sinl(a);
+            }
+            GP_CUDA(cudaMemcpyAsync(c->ztw, w.data(), w.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+            GP_CUDA(cudaStreamSynchronize(c->stream));
+        }
         if (c->zfused) {
             // batched 2-D real transforms over the xy planes; the z direction is zpass.cu's
             int n[2] = {ny, nx}, rembed[2] = {ny, nx}, cembed[2] = {ny, nx / 2 + 1}, pembed[2] = {py, pitch};
@@ -151,14 +170,6 @@ int poisson_setup(gp_ctx* c) {
                 set_error("gp_solve_poisson: cufftPlanMany (inverse, padded output) failed");
                 return GP_ERR_CUFFT;
             }
-            std::vector<double> w(2 * (size_t)nz);
-            for (int k = 0; k < nz; ++k) {
-                const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)nz;
-                w[2 * k] = (double)cosl(a);
-                w[2 * k + 1] = (double)-sinl(a);
-            }
-            GP_CUDA(cudaMemcpyAsync(c->ztw, w.data(), w.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-            GP_CUDA(cudaStreamSynchronize(c->stream));
         } else {
             int n[3] = {nz, ny, nx}, cembed[3] = {nz, ny, nx / 2 + 1}, pembed[3] = {nz + 4, py, pitch};
             GP_CUFFT(cufftPlan3d(&c->plan_fwd, nz, ny, nx, CUFFT_D2Z));
@@ -168,13 +179,6 @@ int poisson_setup(gp_ctx* c) {
                 return GP_ERR_CUFFT;
             }
         }
-        const double pi = 3.14159265358979323846;
-        std::vector<double> t((size_t)nx + ny + nz);
-        for (int k = 0; k < nx; ++k) { const double s = std::sin(pi * k / nx); t[k] = 1.0 - 2.0 / 3.0 * s * s; }
-        for (int k = 0; k < ny; ++k) { const double s = std::sin(pi * k / ny); t[nx + k] = 1.0 - 2.0 / 3.0 * s * s; }
-        for (int k = 0; k < nz; ++k) { const double s = std::sin(pi * k / nz); t[nx + ny + k] = 1.0 - 2.0 / 3.0 * s * s; }
-        GP_CUDA(cudaMemcpyAsync(c->tabx, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-        GP_CUDA(cudaStreamSynchronize(c->stream));
     } else if (c->g.poisson == GP_POISSON_ISOLATED && c->isofast) {
         return iso_pruned_setup(c);
     } else if (c->g.poisson == GP_POISSON_ISOLATED) {

@@ -167,6 +167,10 @@ def test_od_isolated_collapse(pkg, orc):
     check(sim, ref, w, TOL_NSTEP, err_l1)
 
 
+BLK_YY = (slice(0, 2), slice(3, 8), slice(5, 20))       # (z, y, x) blocks of the (32, 12, 10) grid, disjoint from blk
+BLK_ZZ = (slice(2, 6), slice(9, 12), slice(5, 20))
+
+
 def unphysical_state(w):
     """Conserved fields whose total-energy description is NOT physical in a block of cells (rho E - rho v^2/2 < 0,
     n E_xx - n u_x^2 < 0, far from zero), as happens at gas-vacuum borders; the carried fields stay positive."""
@@ -179,6 +183,10 @@ def unphysical_state(w):
         s["E"][blk2] = -0.05                               # even E - rho eps < 0: the velocity is zeroed
     if "Exx" in s:
         s["Exx"][blk] = 0.3 * (s["nux"] ** 2 / s["n"])[blk]
+        # blocks that violate Pi_yy > 0 ALONE and Pi_zz > 0 ALONE (implied value -0.2): all three diagonals of the
+        # condition are exercised (fused_impl.cuh lag epilogue, od.cu k_od_cell)
+        s["Eyy"][BLK_YY] = (s["nuy"] ** 2 / s["n"])[BLK_YY] - 0.2
+        s["Ezz"][BLK_ZZ] = (s["nuz"] ** 2 / s["n"])[BLK_ZZ] - 0.2
     return s
 
 
@@ -211,23 +219,51 @@ def test_balance_alone_on_unphysical_cells(pkg, orc):
     check(sim, ref, w, 1e-14, err_max)
     # all three branches of the gas rule and both of the collisionless rule were taken
     assert np.any(sim.get("mx")[7, 5, 5:20] == 0.0) and np.all(sim.get("E")[7, 5, 5:20] == carried["eps"][7, 5, 5:20])
+    # ... also where Pi_yy or Pi_zz alone is the unphysical one: the carried tensor is kept and all six n E_ij follow it
+    for blk in (BLK_YY, BLK_ZZ):
+        nn, uu = sim.get("n")[blk], [sim.get(k)[blk] / sim.get("n")[blk] for k in ("nux", "nuy", "nuz")]
+        for p, e, (i, j) in zip(PI, ["Exx", "Exy", "Exz", "Eyy", "Eyz", "Ezz"], [(0, 0), (0, 1), (0, 2), (1, 1), (1, 2), (2, 2)]):
+            assert np.array_equal(sim.get(p)[blk], carried[p][blk]), p
+            assert np.abs(sim.get(e)[blk] - (carried[p][blk] + nn * uu[i] * uu[j])).max() <= 1e-14, e
     scale = w.h ** 3 * w.cells
     assert max(sim.kappa()) <= 1e-13 * scale
 
 
 def test_step_with_balance_on_unphysical_cells(pkg, orc):
     """The stages run on the carried (positive) fields where the total-energy description is unphysical, and the
-    balance inside the kernel's epilogue repairs the conserved fields; fixed dt (the CFL reduction of either side
-    rightly reports the unphysical state)."""
+    balance inside the kernel's epilogue repairs the conserved fields; the CFL reduction of an OD context runs on the
+    carried fields as well (reading G16)."""
     w = W.smooth_gas(dims=(32, 12, 10), kmax=2, amp=0.4, components=W.GAS | W.STARS)
     carried = carried_from(w, orc)
     sim, ref = make_pair(pkg, orc, w, perturb=False, state=unphysical_state(w))
     for k, a in carried.items():
         sim.set(k, a)
         ref.set(k, a)
+    # reading G16: in a GP_OD context the CFL reduction takes the carried (positive) fields, so it yields a dt here,
+    # the oracle's; the same state in a base context is rightly reported as unphysical
+    dt_g, dt_r = sim.max_dt(w.cfl), ref.max_dt(w.cfl)
+    assert abs(dt_g - dt_r) <= 1e-13 * dt_r
+    base = pkg.Simulation.from_workload(w)
+    base.set_state(unphysical_state(w))
+    with pytest.raises(pkg.binding.GpError) as e:
+        base.max_dt(w.cfl)
+    assert e.value.code == pkg.binding.GP_ERR_STATE
+    a = carried["Pyy"].copy()
+    a[4, 5, 6] *= -1.0                         # a non-positive CARRIED value is what an OD context reports
+    sim.set("Pyy", a)
     with pytest.raises(pkg.binding.GpError):
         sim.max_dt(w.cfl)
+    sim.set("Pyy", carried["Pyy"])
     dt = 0.05 * w.h
+    # an unbalanced step of a twin pair: the max folded in the kernels' epilogue sees the carried fields too
+    sim2, ref2 = make_pair(pkg, orc, w, perturb=False, state=unphysical_state(w))
+    for k, a in carried.items():
+        sim2.set(k, a)
+        ref2.set(k, a)
+    sim2.od_step(dt, balance=False)
+    ref2.od_step(dt, balance=False)
+    dt_g, dt_r = sim2.max_dt(w.cfl), ref2.max_dt(w.cfl)
+    assert abs(dt_g - dt_r) <= 1e-13 * dt_r
     sim.od_step(dt, balance=True)
     ref.od_step(dt, balance=False)
     k_pre = ref.kappa()                       # what the two stages left, before the balance
@@ -293,3 +329,44 @@ def test_od_fields_round_trip(pkg):
         od.set(k, a)
     for k, a in data.items():
         assert np.array_equal(od.get(k), a), k
+
+
+def test_restart_of_an_od_context_needs_its_carried_fields(pkg, orc):
+    """Restart path: a GP_OD context whose conserved fields were written without the carried ones (or that was never
+    given any) refuses to step, to reduce dt and to balance, instead of running on the pressure of another state;
+    once all fields of the saved state are in, it continues bit for bit like the run it was saved from."""
+    B = pkg.binding
+    w = W.smooth_gas(dims=(24, 12, 10), kmax=2, amp=0.2, components=W.GAS | W.STARS)
+    sim, ref = make_pair(pkg, orc, w)
+    for _ in range(2):
+        od_step(sim, ref, w, False)
+    names = sim.field_names() + sim.od_field_names()
+    saved = {k: sim.get(k) for k in names}
+    fresh = pkg.Simulation(w.nx, w.ny, w.nz, w.h, w.components | GP_OD, w.poisson, w.G, w.gamma, w.bc)
+    for call in (lambda: fresh.od_step(1e-3), lambda: fresh.max_dt(w.cfl), fresh.od_balance, lambda: fresh.step(1e-3)):
+        with pytest.raises(B.GpError) as e:       # fresh storage: no carried fields at all
+            call()
+        assert e.value.code == B.GP_ERR_STATE and "stale" in str(e.value)
+    for k in sim.field_names():
+        fresh.set(k, saved[k])
+    with pytest.raises(B.GpError) as e:           # conserved fields only: still stale
+        fresh.od_step(1e-3, balance=False)
+    assert e.value.code == B.GP_ERR_STATE
+    fresh.set("eps", saved["eps"])
+    with pytest.raises(B.GpError):                # the gas is complete, the collisionless component is not
+        fresh.max_dt(w.cfl)
+    for k in PI:
+        fresh.set(k, saved[k])
+    dt = sim.max_dt(w.cfl)                         # folded by the last step's epilogue
+    dt_fresh = fresh.max_dt(w.cfl)                 # stand-alone reduction over the same state (other rounding of the root)
+    assert abs(dt_fresh - dt) <= 1e-13 * dt
+    fresh.od_step(dt, balance=False)
+    sim.od_step(dt, balance=False)
+    for k in names:
+        assert np.array_equal(fresh.get(k), sim.get(k)), k
+    # writing a conserved field afterwards makes that component's carried fields lag again; gp_od_derive clears it
+    sim.set("rho", sim.get("rho"))
+    with pytest.raises(B.GpError):
+        sim.od_step(dt)
+    sim.od_derive()
+    sim.od_step(dt)
